@@ -1,0 +1,205 @@
+/*
+ * lv.h -- C ABI of the B200-native Langevin droplet step.
+ *
+ * One data-parallel hot path of the model of Derkachov et al. (arxiv
+ * 2501.04456; citations are /root/reference/PAPER.md:<line>): the per-timestep
+ * update of N nanoparticles (NPs) of several coexisting types confined in an
+ * evaporating or condensing spherical microdroplet, PAPER.md:62-69 (sec. 2.2):
+ *   (i)   arrange NPs into cells                         -> hash, sort, cell offsets, scatter
+ *   (ii)  Lennard-Jones + Coulomb pair forces in range   -> pair-force kernel
+ *   (iii) new droplet radius                             -> schedule, on device
+ *   (iv)  surface-tension spring at the interface        \
+ *   (v)   gravity, viscosity, centrifugal                 > fused update kernel
+ *   (vi)  new velocity and position + Brownian kick      /
+ * The formulas (the paper prints none) are the readings R1..R30 of DESIGN.md.
+ *
+ * Conventions
+ *   - Every call returns int: LV_OK (0) or a negative LV_E_* code; nothing is
+ *     printed; no C++ exception crosses this boundary.
+ *   - "host" / "device" is stated for every pointer.  The caller owns every
+ *     buffer it passes; the library owns only the host-side handle and never
+ *     allocates device memory (the caller -- torch -- provides one workspace).
+ *   - All device work is enqueued on the CUDA stream given to lv_bind and runs
+ *     in sm_100a kernels of this library.  There is no CPU fallback.
+ *   - State is fp32; tables are derived on the host in fp64 and rounded once.
+ *   - Call order: lv_create -> lv_set_types [-> lv_set_forces]
+ *     [-> lv_set_droplet_schedule] [-> lv_set_grid] -> lv_workspace_bytes ->
+ *     lv_bind -> lv_set_state -> lv_step / lv_compute_forces / lv_get_* ...
+ *     -> lv_destroy.  A setter called after lv_bind returns LV_E_ORDER.
+ */
+#ifndef LV_H_
+#define LV_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define LV_MAX_TYPES 8
+
+/* return codes */
+#define LV_OK            0
+#define LV_E_ARG        -1   /* bad argument */
+#define LV_E_ORDER      -2   /* call order violated */
+#define LV_E_WORKSPACE  -3   /* workspace too small or misaligned (256 B) */
+#define LV_E_CUDA       -4   /* a CUDA runtime call failed; see lv_last_cuda_error */
+#define LV_E_NONFINITE  -5   /* sticky: a non-finite position or velocity appeared (R6) */
+#define LV_E_NOMEM      -6   /* host allocation failed */
+
+/* droplet schedule modes: step (iii); radius-square law PAPER.md:58 */
+#define LV_SCHED_CONST   0
+#define LV_SCHED_LINEAR  1   /* R linear in the step index */
+#define LV_SCHED_R2LAW   2   /* R^2 linear in the step index */
+
+/* surface force modes: step (iv) */
+#define LV_WALL_ONESIDED 0   /* spring for every pen > 0 (R7) */
+#define LV_WALL_WINDOW   1   /* only while 0 < pen < 2 r_NP: the paper's (-r_NP, r_NP) window */
+
+/* status bits (lv_get_status); warnings do not stop the simulation */
+#define LV_ST_NONFINITE    1u   /* error: also returned as LV_E_NONFINITE */
+#define LV_ST_OUTSIDE_GRID 2u   /* warning: an NP was clamped into a border cell (R22) */
+
+/* lv_get_debug selectors (parity tests) */
+#define LV_DBG_KEYS          1  /* uint32[N]   cell key per slot before the sort            */
+#define LV_DBG_KEYS_SORTED   2  /* uint32[N]                                                */
+#define LV_DBG_PERM          3  /* uint32[N]   sorted slot k came from slot perm[k]         */
+#define LV_DBG_CELL_OFFSETS  4  /* uint32[n_cells+1] cell c holds sorted slots [off[c], off[c+1]) */
+#define LV_DBG_IDS_SORTED    5  /* uint32[N]   NP id at each sorted slot                    */
+#define LV_DBG_GRID          6  /* lv_grid_info (host struct only)                          */
+
+typedef struct lv_sim lv_sim;   /* opaque, host memory, owned by the library */
+
+/* One NP type, PAPER.md:58 ("radius, mass, charge"; per-type spring constant;
+ * kick magnitude "passed as a parameter"). */
+typedef struct {
+    double sigma;    /* NP diameter; r_NP = sigma/2                                   */
+    double eps;      /* LJ well depth of the type (used only when eps_TxT == NULL)    */
+    double mass;
+    double charge;
+    double wall_k;   /* surface spring constant                                       */
+    double drag_a;   /* velocity retained per step, a = 1 - gamma dt (R11)            */
+    double kick_b;   /* std of each component of the random velocity added per step   */
+} lv_type;
+
+/* The grids the cell list uses, as exact fp32/fp64 values (LV_DBG_GRID). */
+typedef struct {
+    int32_t  n_types;
+    int32_t  G[LV_MAX_TYPES];           /* cells per axis of the grid of type b        */
+    uint32_t base[LV_MAX_TYPES + 1];    /* first key of grid b; base[n_types] = cells  */
+    float    lo[LV_MAX_TYPES];          /* lower corner on every axis                  */
+    float    inv_h[LV_MAX_TYPES];
+    double   h[LV_MAX_TYPES];           /* cell edge                                   */
+    int32_t  w[LV_MAX_TYPES * LV_MAX_TYPES]; /* stencil half-width, [a*LV_MAX_TYPES+b] */
+} lv_grid_info;
+
+/* a = 1 - gamma dt, b = sqrt((kT/m)(1 - a^2)): explicit Stokes drag and the
+ * kick that keeps <v^2> = kT/m stationary (R11, R15).
+ * a, b: host, written. */
+int lv_langevin_coeffs(double gamma, double kT, double mass, double dt, double *a, double *b);
+
+/* Allocate a handle (host) for n NPs of n_types types (1..LV_MAX_TYPES).
+ * seed keys the Philox4x32-10 noise (R15); dt is the time step. */
+int lv_create(lv_sim **out, int n, int n_types, uint64_t seed, double dt);
+
+/* NP types and the type x type interaction tables (interactions
+ * "within each NP type and between types can be freely set").  All host,
+ * copied.  types[n_types].  eps_TxT / sigma_TxT / rcut_TxT: row-major
+ * [n_types*n_types] or NULL; NULL -> Lorentz-Berthelot eps_ab = sqrt(eps_a
+ * eps_b), sigma_ab = (sigma_a + sigma_b)/2 (= r_A + r_B),
+ * r_c,ab = cut_factor * sigma_ab (4 (r_A + r_B) in the paper's
+ * runs).  coulomb_k is k_C in U = k_C q_a q_b / r (R5).  Both potentials are
+ * truncated at r_c,ab and NOT shifted.  Tables must be
+ * symmetric. */
+int lv_set_types(lv_sim *s, int n_types, const lv_type *types, const double *eps_TxT,
+                 const double *sigma_TxT, const double *rcut_TxT, double cut_factor,
+                 double coulomb_k);
+
+/* External fields, step (v) PAPER.md:68: gravity g along -z,
+ * centrifugal force m (omega2_xyz[0] x, omega2_xyz[1] y, omega2_xyz[2] z)
+ * (isotropic tumbling = (w^2,w^2,w^2); rotation about z = (w^2,w^2,0)), and the
+ * surface-force mode.  omega2_xyz: host[3].  Default: 0, (0,0,0), ONESIDED. */
+int lv_set_forces(lv_sim *s, double g, const double *omega2_xyz, int wall_mode);
+
+/* Droplet radius as a function of the integer step index n (step (iii),
+ * PAPER.md:66): f = min(n, n_steps)/n_steps; CONST R0; LINEAR R0 + (R1-R0) f;
+ * R2LAW sqrt(R0^2 + (R1^2-R0^2) f).  R1 > R0 is condensation.
+ * During step n the surface stands at R(n+1) (R9). */
+int lv_set_droplet_schedule(lv_sim *s, int mode, double R0, double R1, int64_t n_steps);
+
+/* Optional: cells per cut-off k_b >= 1 for the grid of each type (host
+ * [n_types]); cell edge h_b = r_c,bb (1 + 2^-9) / k_b.  Default 1. */
+int lv_set_grid(lv_sim *s, const int32_t *cells_per_cut);
+
+/* Bytes of device workspace lv_bind needs (0 if types are not set). */
+size_t lv_workspace_bytes(const lv_sim *s);
+
+/* Freeze the configuration, carve the caller's device workspace (device
+ * pointer, 256-byte aligned, >= lv_workspace_bytes, owned by the caller and
+ * kept alive until lv_destroy) and remember the CUDA stream (a cudaStream_t
+ * passed as void*; NULL = the legacy default stream). */
+int lv_bind(lv_sim *s, void *workspace_dev, size_t workspace_bytes, void *cuda_stream);
+
+/* Load a configuration (also the restart path).  pos_xyz,
+ * vel_xyz: [n][3] fp32; type: [n] int32 in [0, n_types); all three host
+ * (on_device = 0) or all device (on_device = 1); copied.  NP id = row index.
+ * step = index of the next step to take.  Synchronises the stream when the
+ * sources are host buffers. */
+int lv_set_state(lv_sim *s, const float *pos_xyz, const float *vel_xyz, const int32_t *type,
+                 int64_t step, int on_device);
+
+/* Enqueue n full steps on the stream and return without
+ * synchronising.  lv_step(a); lv_step(b) equals lv_step(a + b) bit for bit. */
+int lv_step(lv_sim *s, int n);
+
+/* Steps (i)-(ii) only on the current state: rebuild the cell structures and
+ * compute the pair forces; the state does not change.  Asynchronous. */
+int lv_compute_forces(lv_sim *s);
+
+/* Write the state in NP-id order into caller buffers ([n][3] fp32, [n] int32;
+ * host or device per on_device; any pointer may be NULL), R = droplet radius
+ * R(step) and step (host, may be NULL).  Synchronises the stream.  Returns
+ * LV_E_NONFINITE if the sticky error bit is set. */
+int lv_get_state(lv_sim *s, float *pos_xyz, float *vel_xyz, int32_t *type, double *R,
+                 int64_t *step, int on_device);
+
+/* Pair forces of the last lv_compute_forces / lv_step in NP-id order:
+ * force_xyz [n][3] fp32 and neigh_count [n] int32 (NPs inside r_c,ab); host or
+ * device per on_device; either may be NULL.  Synchronises. */
+int lv_get_forces(lv_sim *s, float *force_xyz, int32_t *neigh_count, int on_device);
+
+/* Status bits LV_ST_* (host uint32, written).  Synchronises. */
+int lv_get_status(lv_sim *s, uint32_t *status);
+
+/* Internal arrays for parity tests: copies min(bytes, size of the array) bytes
+ * of the array `what` (LV_DBG_*) to dst (host, or device if on_device).
+ * The arrays describe the last cell rebuild.  Synchronises. */
+int lv_get_debug(lv_sim *s, int what, void *dst, size_t bytes, int on_device);
+
+/* Number of kernels (own + CUB sort) one lv_step(1) enqueues; for accounting. */
+int lv_launches_per_step(const lv_sim *s);
+
+/* Measurement aid: take ONE step exactly like lv_step(1) (same kernels, direct
+ * launches instead of the graph) with CUDA events between the stages on the
+ * stream, synchronise, and write the device time of each stage in
+ * milliseconds to ms_out (host[LV_N_STAGES]): hash, sort, offsets+scatter,
+ * pair force, update. */
+#define LV_N_STAGES 5
+int lv_step_profiled(lv_sim *s, float *ms_out);
+
+/* Measurement aid: FP32 FMA throughput of this GPU from a register-resident
+ * independent-FMA kernel on `cuda_stream`; writes TFLOP/s (host).  The
+ * denominator of the pair-force kernel's ALU roofline. */
+int lv_measure_fp32_peak(void *cuda_stream, double *tflops);
+
+int lv_destroy(lv_sim *s);
+const char *lv_strerror(int code);
+/* Text of the last CUDA error seen by this handle (host string, library-owned). */
+const char *lv_last_cuda_error(const lv_sim *s);
+const char *lv_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LV_H_ */

@@ -1,0 +1,593 @@
+// lv_api.cu -- the C ABI of include/lv.h: host-side handle, derivation of the
+// fp32 tables (fp64 -> fp32 once), workspace carving, CUDA-graph capture of one
+// step and the state / debug accessors.  Every step of the path runs in the
+// kernels of lv_kernels.cu / lv_sort.cu; there is no CPU fallback.
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+
+#include "lv_internal.cuh"
+
+struct lv_sim {
+    int n = 0, n_types = 0;
+    uint64_t seed = 0;
+    double dt = 0.0;
+    bool types_set = false, sched_set = false, bound = false, state_set = false;
+    lv_type types[LV_MAX_TYPES];
+    double eps[LV_MAX_TYPES * LV_MAX_TYPES];
+    double sig[LV_MAX_TYPES * LV_MAX_TYPES];
+    double rcut[LV_MAX_TYPES * LV_MAX_TYPES];
+    double coulomb_k = 0.0;
+    double g = 0.0;
+    double om2[3] = {0.0, 0.0, 0.0};
+    int wall_mode = LV_WALL_ONESIDED;
+    int sched_mode = LV_SCHED_CONST;
+    double R0 = 0.0, R1 = 0.0;
+    int64_t sched_steps = 0;
+    int32_t cells_per_cut[LV_MAX_TYPES];
+    lv_grid_info grid;
+    int sort_end_bit = 1;
+    size_t ws_bytes = 0;
+    LvDev dev;
+    LvBufs bufs;
+    cudaStream_t stream = nullptr;
+    cudaGraph_t graph = nullptr;
+    cudaGraphExec_t graph_exec = nullptr;
+    int launches_per_step = 0;
+    char cuda_err[256];
+};
+
+namespace {
+
+constexpr size_t kAlign = 256;
+inline size_t align_up(size_t x) { return (x + kAlign - 1) / kAlign * kAlign; }
+
+int cuda_fail(lv_sim *s, cudaError_t e, const char *where)
+{
+    snprintf(s->cuda_err, sizeof(s->cuda_err), "%s: %s", where, cudaGetErrorString(e));
+    return LV_E_CUDA;
+}
+#define LV_CUDA(s, call)                                        \
+    do {                                                        \
+        cudaError_t e_ = (call);                                \
+        if (e_ != cudaSuccess) return cuda_fail((s), e_, #call); \
+    } while (0)
+
+// DESIGN.md "Grid rule" (restated independently of the oracle): one grid per NP
+// type b, h_b = r_c,bb (1 + 2^-9) / k_b, covering the largest droplet plus one
+// largest NP diameter; stencil half-width w_ab = ceil(r_c,ab (1 + 2^-10) / h_b).
+int derive_grid(lv_sim *s)
+{
+    const int T = s->n_types;
+    const double Rmax = s->sched_mode == LV_SCHED_CONST ? s->R0 : std::fmax(s->R0, s->R1);
+    double smax = 0.0;
+    for (int a = 0; a < T; ++a) smax = std::fmax(smax, s->types[a].sigma);
+    lv_grid_info &g = s->grid;
+    memset(&g, 0, sizeof(g));
+    g.n_types = T;
+    uint64_t base = 0;
+    for (int b = 0; b < T; ++b) {
+        const double h = s->rcut[b * LV_MAX_TYPES + b] * (1.0 + 1.0 / 512.0) / (double)s->cells_per_cut[b];
+        const double Gd = std::ceil((2.0 * Rmax + 2.0 * smax) / h);
+        if (!(Gd >= 1.0) || Gd > 1600.0) return LV_E_ARG;
+        const int G = (int)Gd;
+        g.h[b] = h;
+        g.G[b] = G;
+        g.lo[b] = (float)(-0.5 * (double)G * h);
+        g.inv_h[b] = (float)(1.0 / h);
+        g.base[b] = (uint32_t)base;
+        base += (uint64_t)G * G * G;
+        if (base > (1ull << 30)) return LV_E_ARG;
+    }
+    g.base[T] = (uint32_t)base;
+    for (int a = 0; a < T; ++a)
+        for (int b = 0; b < T; ++b) {
+            const double w = std::ceil(s->rcut[a * LV_MAX_TYPES + b] * (1.0 + 1.0 / 1024.0) / g.h[b]);
+            if (w > 100.0) return LV_E_ARG;
+            g.w[a * LV_MAX_TYPES + b] = (int32_t)w;
+        }
+    int bits = 1;
+    while (bits < 32 && (1ull << bits) < base) ++bits;
+    s->sort_end_bit = bits;
+    return LV_OK;
+}
+
+struct Layout {
+    size_t posA, velA, posB, velB, force, key_in, key_out, val_in, val_out, cell_off, sort_temp,
+        sort_temp_bytes, st, staging, total;
+};
+
+Layout layout_of(const lv_sim *s)
+{
+    Layout L;
+    const size_t n = (size_t)(s->n > 0 ? s->n : 1);
+    size_t o = 0;
+    auto take = [&](size_t bytes) { size_t at = o; o = align_up(o + bytes); return at; };
+    L.posA = take(16 * n); L.velA = take(16 * n);
+    L.posB = take(16 * n); L.velB = take(16 * n);
+    L.force = take(16 * n);
+    L.key_in = take(4 * n); L.key_out = take(4 * n);
+    L.val_in = take(4 * n); L.val_out = take(4 * n);
+    L.cell_off = take(4 * ((size_t)s->grid.base[s->n_types] + 1));
+    L.sort_temp_bytes = lvs_temp_bytes(s->n, s->sort_end_bit);
+    L.sort_temp = take(L.sort_temp_bytes);
+    L.st = take(sizeof(LvDevState));
+    L.staging = take(28 * n);
+    L.total = o;
+    return L;
+}
+
+void derive_tables(lv_sim *s)
+{
+    LvDev &d = s->dev;
+    memset(&d, 0, sizeof(d));
+    const int T = s->n_types;
+    d.n = s->n;
+    d.n_types = T;
+    d.n_cells = s->grid.base[T];
+    d.wall_mode = s->wall_mode;
+    for (int a = 0; a < T; ++a)
+        for (int b = 0; b < T; ++b) {
+            const int k = a * LV_MAX_TYPES + b;
+            const double sg = s->sig[k], s6 = sg * sg * sg * sg * sg * sg;
+            d.pair[k].rc2 = (float)(s->rcut[k] * s->rcut[k]);
+            d.pair[k].c12 = (float)(48.0 * s->eps[k] * s6 * s6);
+            d.pair[k].c6 = (float)(24.0 * s->eps[k] * s6);
+            d.pair[k].qq = (float)(s->coulomb_k * s->types[a].charge * s->types[b].charge);
+            d.w[k] = (int8_t)s->grid.w[k];
+        }
+    for (int a = 0; a < T; ++a) {
+        const lv_type &t = s->types[a];
+        d.type[a].dt_over_m = (float)(s->dt / t.mass);
+        d.type[a].a = (float)t.drag_a;
+        d.type[a].b = (float)t.kick_b;
+        d.type[a].mass = (float)t.mass;
+        d.type[a].radius = (float)(0.5 * t.sigma);
+        d.wall_k_d[a] = t.wall_k;
+        d.radius_d[a] = 0.5 * t.sigma;
+        d.grid[a].lo = s->grid.lo[a];
+        d.grid[a].inv_h = s->grid.inv_h[a];
+        d.grid[a].G = s->grid.G[a];
+        d.grid[a].base = s->grid.base[a];
+    }
+    d.dt = (float)s->dt;
+    d.g = (float)s->g;
+    for (int k = 0; k < 3; ++k) d.om2[k] = (float)s->om2[k];
+    d.sched_mode = s->sched_mode;
+    d.sched_steps = s->sched_steps;
+    d.R0 = s->R0;
+    d.R1 = s->R1;
+    d.seed_lo = (uint32_t)s->seed;
+    d.seed_hi = (uint32_t)(s->seed >> 32);
+}
+
+// steps (i)-(ii): hash -> sort -> offsets + scatter -> pair force
+int enqueue_rebuild_and_forces(lv_sim *s)
+{
+    LV_CUDA(s, lvk_hash(s->dev, s->bufs, s->stream));
+    LV_CUDA(s, lvs_sort_pairs(s->bufs.sort_temp, s->bufs.sort_temp_bytes, s->bufs.key_in,
+                              s->bufs.key_out, s->bufs.val_in, s->bufs.val_out, s->n,
+                              s->sort_end_bit, s->stream));
+    LV_CUDA(s, lvk_bounds_scatter(s->dev, s->bufs, s->stream));
+    LV_CUDA(s, lvk_pair_force(s->dev, s->bufs, s->stream));
+    return LV_OK;
+}
+
+int enqueue_step(lv_sim *s)
+{
+    int rc = enqueue_rebuild_and_forces(s);
+    if (rc != LV_OK) return rc;
+    LV_CUDA(s, lvk_update(s->dev, s->bufs, s->stream));
+    return LV_OK;
+}
+
+// Capture one step into a graph (nothing executes during capture).  The graph
+// is static: the step index and the radius live in device memory.
+int build_graph(lv_sim *s)
+{
+    if (s->stream == nullptr || s->n == 0) return LV_OK;   // legacy stream: direct launches
+    LV_CUDA(s, cudaStreamBeginCapture(s->stream, cudaStreamCaptureModeRelaxed));
+    int rc = enqueue_step(s);
+    cudaGraph_t g = nullptr;
+    cudaError_t e = cudaStreamEndCapture(s->stream, &g);
+    if (rc != LV_OK) { if (g) cudaGraphDestroy(g); return rc; }
+    if (e != cudaSuccess) return cuda_fail(s, e, "cudaStreamEndCapture");
+    s->graph = g;
+    size_t nn = 0;
+    LV_CUDA(s, cudaGraphGetNodes(g, nullptr, &nn));
+    cudaGraphNode_t *nodes = (cudaGraphNode_t *)malloc(sizeof(cudaGraphNode_t) * (nn ? nn : 1));
+    if (!nodes) return LV_E_NOMEM;
+    cudaError_t e2 = cudaGraphGetNodes(g, nodes, &nn);
+    int kernels = 0;
+    for (size_t i = 0; e2 == cudaSuccess && i < nn; ++i) {
+        cudaGraphNodeType t;
+        if (cudaGraphNodeGetType(nodes[i], &t) == cudaSuccess && t == cudaGraphNodeTypeKernel) ++kernels;
+    }
+    free(nodes);
+    if (e2 != cudaSuccess) return cuda_fail(s, e2, "cudaGraphGetNodes");
+    s->launches_per_step = kernels;
+    LV_CUDA(s, cudaGraphInstantiate(&s->graph_exec, g, 0));
+    return LV_OK;
+}
+
+int copy_out(lv_sim *s, void *dst, const void *src_dev, size_t bytes, int on_device)
+{
+    LV_CUDA(s, cudaMemcpyAsync(dst, src_dev, bytes,
+                               on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, s->stream));
+    return LV_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int lv_langevin_coeffs(double gamma, double kT, double mass, double dt, double *a, double *b)
+{
+    if (!a || !b || !(mass > 0.0) || !(dt > 0.0) || !(kT >= 0.0) || !(gamma >= 0.0)) return LV_E_ARG;
+    *a = 1.0 - gamma * dt;
+    *b = std::sqrt((kT / mass) * (1.0 - (*a) * (*a)));
+    return LV_OK;
+}
+
+int lv_create(lv_sim **out, int n, int n_types, uint64_t seed, double dt)
+{
+    if (!out || n < 0 || n_types < 1 || n_types > LV_MAX_TYPES || !(dt > 0.0)) return LV_E_ARG;
+    lv_sim *s = new (std::nothrow) lv_sim();
+    if (!s) return LV_E_NOMEM;
+    s->n = n;
+    s->n_types = n_types;
+    s->seed = seed;
+    s->dt = dt;
+    for (int b = 0; b < LV_MAX_TYPES; ++b) s->cells_per_cut[b] = 1;
+    s->cuda_err[0] = 0;
+    memset(&s->bufs, 0, sizeof(s->bufs));
+    *out = s;
+    return LV_OK;
+}
+
+int lv_set_types(lv_sim *s, int n_types, const lv_type *types, const double *eps_TxT,
+                 const double *sigma_TxT, const double *rcut_TxT, double cut_factor, double coulomb_k)
+{
+    if (!s || !types || n_types != s->n_types) return LV_E_ARG;
+    if (s->bound) return LV_E_ORDER;
+    const int T = n_types;
+    for (int a = 0; a < T; ++a) {
+        const lv_type &t = types[a];
+        if (!(t.sigma > 0.0) || !(t.mass > 0.0) || !(t.wall_k >= 0.0) || !(t.kick_b >= 0.0) ||
+            !std::isfinite(t.charge) || !std::isfinite(t.drag_a) || !(t.eps >= 0.0))
+            return LV_E_ARG;
+    }
+    if (!rcut_TxT && !(cut_factor > 0.0)) return LV_E_ARG;
+    for (int a = 0; a < T; ++a)
+        for (int b = 0; b < T; ++b) {
+            const int k = a * LV_MAX_TYPES + b, u = a * T + b, ut = b * T + a;
+            const double sg = sigma_TxT ? sigma_TxT[u] : 0.5 * types[a].sigma + 0.5 * types[b].sigma;
+            const double ep = eps_TxT ? eps_TxT[u] : std::sqrt(types[a].eps * types[b].eps);
+            const double rc = rcut_TxT ? rcut_TxT[u] : cut_factor * sg;
+            if (!(sg > 0.0) || !(ep >= 0.0) || !(rc > 0.0)) return LV_E_ARG;
+            if ((sigma_TxT && sigma_TxT[u] != sigma_TxT[ut]) || (eps_TxT && eps_TxT[u] != eps_TxT[ut]) ||
+                (rcut_TxT && rcut_TxT[u] != rcut_TxT[ut]))
+                return LV_E_ARG;
+            s->sig[k] = sg;
+            s->eps[k] = ep;
+            s->rcut[k] = rc;
+        }
+    memcpy(s->types, types, sizeof(lv_type) * T);
+    s->coulomb_k = coulomb_k;
+    s->types_set = true;
+    return LV_OK;
+}
+
+int lv_set_forces(lv_sim *s, double g, const double *omega2_xyz, int wall_mode)
+{
+    if (!s || !std::isfinite(g) || (wall_mode != LV_WALL_ONESIDED && wall_mode != LV_WALL_WINDOW))
+        return LV_E_ARG;
+    if (s->bound) return LV_E_ORDER;
+    s->g = g;
+    for (int k = 0; k < 3; ++k) s->om2[k] = omega2_xyz ? omega2_xyz[k] : 0.0;
+    s->wall_mode = wall_mode;
+    return LV_OK;
+}
+
+int lv_set_droplet_schedule(lv_sim *s, int mode, double R0, double R1, int64_t n_steps)
+{
+    if (!s || mode < LV_SCHED_CONST || mode > LV_SCHED_R2LAW || !(R0 > 0.0)) return LV_E_ARG;
+    if (mode != LV_SCHED_CONST && (!(R1 > 0.0) || n_steps < 1)) return LV_E_ARG;
+    if (s->bound) return LV_E_ORDER;
+    s->sched_mode = mode;
+    s->R0 = R0;
+    s->R1 = mode == LV_SCHED_CONST ? R0 : R1;
+    s->sched_steps = mode == LV_SCHED_CONST ? 0 : n_steps;
+    s->sched_set = true;
+    return LV_OK;
+}
+
+int lv_set_grid(lv_sim *s, const int32_t *cells_per_cut)
+{
+    if (!s || !cells_per_cut) return LV_E_ARG;
+    if (s->bound) return LV_E_ORDER;
+    for (int b = 0; b < s->n_types; ++b)
+        if (cells_per_cut[b] < 1 || cells_per_cut[b] > 16) return LV_E_ARG;
+    for (int b = 0; b < s->n_types; ++b) s->cells_per_cut[b] = cells_per_cut[b];
+    return LV_OK;
+}
+
+size_t lv_workspace_bytes(const lv_sim *cs)
+{
+    lv_sim *s = const_cast<lv_sim *>(cs);
+    if (!s || !s->types_set || !s->sched_set) return 0;
+    if (derive_grid(s) != LV_OK) return 0;
+    return layout_of(s).total;
+}
+
+int lv_bind(lv_sim *s, void *workspace_dev, size_t workspace_bytes, void *cuda_stream)
+{
+    if (!s) return LV_E_ARG;
+    if (!s->types_set || !s->sched_set) return LV_E_ORDER;
+    if (s->bound) return LV_E_ORDER;
+    int rc = derive_grid(s);
+    if (rc != LV_OK) return rc;
+    const Layout L = layout_of(s);
+    if (!workspace_dev || workspace_bytes < L.total || ((uintptr_t)workspace_dev % kAlign) != 0)
+        return LV_E_WORKSPACE;
+    unsigned char *w = (unsigned char *)workspace_dev;
+    LvBufs &B = s->bufs;
+    B.posA = (float4 *)(w + L.posA); B.velA = (float4 *)(w + L.velA);
+    B.posB = (float4 *)(w + L.posB); B.velB = (float4 *)(w + L.velB);
+    B.force = (float4 *)(w + L.force);
+    B.key_in = (uint32_t *)(w + L.key_in); B.key_out = (uint32_t *)(w + L.key_out);
+    B.val_in = (uint32_t *)(w + L.val_in); B.val_out = (uint32_t *)(w + L.val_out);
+    B.cell_off = (uint32_t *)(w + L.cell_off);
+    B.sort_temp = w + L.sort_temp;
+    B.sort_temp_bytes = L.sort_temp_bytes;
+    B.st = (LvDevState *)(w + L.st);
+    B.staging = w + L.staging;
+    s->ws_bytes = L.total;
+    s->stream = (cudaStream_t)cuda_stream;
+    derive_tables(s);
+    LV_CUDA(s, cudaMemsetAsync(B.st, 0, sizeof(LvDevState), s->stream));
+    rc = build_graph(s);
+    if (rc != LV_OK) return rc;
+    s->bound = true;
+    return LV_OK;
+}
+
+int lv_set_state(lv_sim *s, const float *pos_xyz, const float *vel_xyz, const int32_t *type,
+                 int64_t step, int on_device)
+{
+    if (!s || step < 0) return LV_E_ARG;
+    if (!s->bound) return LV_E_ORDER;
+    if (s->n > 0 && (!pos_xyz || !vel_xyz || !type)) return LV_E_ARG;
+    const size_t n = (size_t)s->n;
+    const float *dp = pos_xyz, *dv = vel_xyz;
+    const int32_t *dt = type;
+    if (!on_device && n > 0) {
+        unsigned char *stg = s->bufs.staging;
+        LV_CUDA(s, cudaMemcpyAsync(stg, pos_xyz, 12 * n, cudaMemcpyHostToDevice, s->stream));
+        LV_CUDA(s, cudaMemcpyAsync(stg + 12 * n, vel_xyz, 12 * n, cudaMemcpyHostToDevice, s->stream));
+        LV_CUDA(s, cudaMemcpyAsync(stg + 24 * n, type, 4 * n, cudaMemcpyHostToDevice, s->stream));
+        dp = (const float *)stg;
+        dv = (const float *)(stg + 12 * n);
+        dt = (const int32_t *)(stg + 24 * n);
+    }
+    LV_CUDA(s, lvk_pack_state(s->dev, s->bufs, dp, dv, dt, (long long)step, s->stream));
+    if (!on_device) LV_CUDA(s, cudaStreamSynchronize(s->stream));
+    s->state_set = true;
+    return LV_OK;
+}
+
+int lv_step(lv_sim *s, int n)
+{
+    if (!s || n < 0) return LV_E_ARG;
+    if (!s->bound || !s->state_set) return LV_E_ORDER;
+    if (s->n == 0) return LV_OK;
+    for (int k = 0; k < n; ++k) {
+        if (s->graph_exec) {
+            LV_CUDA(s, cudaGraphLaunch(s->graph_exec, s->stream));
+        } else {
+            int rc = enqueue_step(s);
+            if (rc != LV_OK) return rc;
+        }
+    }
+    return LV_OK;
+}
+
+int lv_compute_forces(lv_sim *s)
+{
+    if (!s) return LV_E_ARG;
+    if (!s->bound || !s->state_set) return LV_E_ORDER;
+    if (s->n == 0) return LV_OK;
+    return enqueue_rebuild_and_forces(s);
+}
+
+int lv_get_status(lv_sim *s, uint32_t *status)
+{
+    if (!s || !status) return LV_E_ARG;
+    if (!s->bound) return LV_E_ORDER;
+    LvDevState h;
+    LV_CUDA(s, cudaMemcpyAsync(&h, s->bufs.st, sizeof(h), cudaMemcpyDeviceToHost, s->stream));
+    LV_CUDA(s, cudaStreamSynchronize(s->stream));
+    *status = h.status;
+    return LV_OK;
+}
+
+int lv_get_state(lv_sim *s, float *pos_xyz, float *vel_xyz, int32_t *type, double *R, int64_t *step,
+                 int on_device)
+{
+    if (!s) return LV_E_ARG;
+    if (!s->bound || !s->state_set) return LV_E_ORDER;
+    const size_t n = (size_t)s->n;
+    if (n > 0 && (pos_xyz || vel_xyz || type)) {
+        if (on_device) {
+            LV_CUDA(s, lvk_unpack_state(s->dev, s->bufs, pos_xyz, vel_xyz, type, s->stream));
+        } else {
+            unsigned char *stg = s->bufs.staging;
+            float *dp = (float *)stg, *dv = (float *)(stg + 12 * n);
+            int32_t *dt = (int32_t *)(stg + 24 * n);
+            LV_CUDA(s, lvk_unpack_state(s->dev, s->bufs, pos_xyz ? dp : nullptr, vel_xyz ? dv : nullptr,
+                                        type ? dt : nullptr, s->stream));
+            if (pos_xyz) LV_CUDA(s, cudaMemcpyAsync(pos_xyz, dp, 12 * n, cudaMemcpyDeviceToHost, s->stream));
+            if (vel_xyz) LV_CUDA(s, cudaMemcpyAsync(vel_xyz, dv, 12 * n, cudaMemcpyDeviceToHost, s->stream));
+            if (type) LV_CUDA(s, cudaMemcpyAsync(type, dt, 4 * n, cudaMemcpyDeviceToHost, s->stream));
+        }
+    }
+    LvDevState h;
+    LV_CUDA(s, cudaMemcpyAsync(&h, s->bufs.st, sizeof(h), cudaMemcpyDeviceToHost, s->stream));
+    LV_CUDA(s, cudaStreamSynchronize(s->stream));
+    if (step) *step = (int64_t)h.step;
+    if (R) *R = lv_radius_of(s->sched_mode, s->R0, s->R1, s->sched_steps, h.step);
+    return (h.status & LV_ST_NONFINITE) ? LV_E_NONFINITE : LV_OK;
+}
+
+int lv_get_forces(lv_sim *s, float *force_xyz, int32_t *neigh_count, int on_device)
+{
+    if (!s) return LV_E_ARG;
+    if (!s->bound || !s->state_set) return LV_E_ORDER;
+    const size_t n = (size_t)s->n;
+    if (n > 0 && (force_xyz || neigh_count)) {
+        if (on_device) {
+            LV_CUDA(s, lvk_unpack_forces(s->dev, s->bufs, force_xyz, neigh_count, s->stream));
+        } else {
+            unsigned char *stg = s->bufs.staging;
+            float *df = (float *)stg;
+            int32_t *dc = (int32_t *)(stg + 12 * n);
+            LV_CUDA(s, lvk_unpack_forces(s->dev, s->bufs, force_xyz ? df : nullptr,
+                                         neigh_count ? dc : nullptr, s->stream));
+            if (force_xyz) LV_CUDA(s, cudaMemcpyAsync(force_xyz, df, 12 * n, cudaMemcpyDeviceToHost, s->stream));
+            if (neigh_count) LV_CUDA(s, cudaMemcpyAsync(neigh_count, dc, 4 * n, cudaMemcpyDeviceToHost, s->stream));
+        }
+    }
+    LV_CUDA(s, cudaStreamSynchronize(s->stream));
+    return LV_OK;
+}
+
+int lv_get_debug(lv_sim *s, int what, void *dst, size_t bytes, int on_device)
+{
+    if (!s || !dst) return LV_E_ARG;
+    if (what == LV_DBG_GRID) {   // host-only: available as soon as types and schedule are set
+        if (on_device) return LV_E_ARG;
+        if (!s->types_set || !s->sched_set) return LV_E_ORDER;
+        if (!s->bound) { int rg = derive_grid(s); if (rg != LV_OK) return rg; }
+        memcpy(dst, &s->grid, bytes < sizeof(lv_grid_info) ? bytes : sizeof(lv_grid_info));
+        return LV_OK;
+    }
+    if (!s->bound) return LV_E_ORDER;
+    const size_t n = (size_t)s->n;
+    int rc = LV_OK;
+    switch (what) {
+    case LV_DBG_KEYS:
+        rc = copy_out(s, dst, s->bufs.key_in, bytes < 4 * n ? bytes : 4 * n, on_device); break;
+    case LV_DBG_KEYS_SORTED:
+        rc = copy_out(s, dst, s->bufs.key_out, bytes < 4 * n ? bytes : 4 * n, on_device); break;
+    case LV_DBG_PERM:
+        rc = copy_out(s, dst, s->bufs.val_out, bytes < 4 * n ? bytes : 4 * n, on_device); break;
+    case LV_DBG_CELL_OFFSETS: {
+        const size_t full = 4 * ((size_t)s->grid.base[s->n_types] + 1);
+        rc = copy_out(s, dst, s->bufs.cell_off, bytes < full ? bytes : full, on_device); break;
+    }
+    case LV_DBG_IDS_SORTED:
+        if (n == 0) break;
+        LV_CUDA(s, lvk_ids_sorted(s->dev, s->bufs, (uint32_t *)s->bufs.staging, s->stream));
+        rc = copy_out(s, dst, s->bufs.staging, bytes < 4 * n ? bytes : 4 * n, on_device); break;
+    default:
+        return LV_E_ARG;
+    }
+    if (rc != LV_OK) return rc;
+    LV_CUDA(s, cudaStreamSynchronize(s->stream));
+    return LV_OK;
+}
+
+int lv_launches_per_step(const lv_sim *s) { return s ? s->launches_per_step : 0; }
+
+int lv_step_profiled(lv_sim *s, float *ms_out)
+{
+    if (!s || !ms_out) return LV_E_ARG;
+    if (!s->bound || !s->state_set) return LV_E_ORDER;
+    for (int k = 0; k < LV_N_STAGES; ++k) ms_out[k] = 0.f;
+    if (s->n == 0) return LV_OK;
+    cudaEvent_t ev[LV_N_STAGES + 1];
+    for (int k = 0; k <= LV_N_STAGES; ++k) LV_CUDA(s, cudaEventCreate(&ev[k]));
+    int rc = LV_OK;
+    cudaError_t e = cudaSuccess;
+#define LV_STAGE(k, call)                                         \
+    if (e == cudaSuccess) e = (call);                             \
+    if (e == cudaSuccess) e = cudaEventRecord(ev[(k) + 1], s->stream);
+    e = cudaEventRecord(ev[0], s->stream);
+    LV_STAGE(0, lvk_hash(s->dev, s->bufs, s->stream));
+    LV_STAGE(1, lvs_sort_pairs(s->bufs.sort_temp, s->bufs.sort_temp_bytes, s->bufs.key_in,
+                               s->bufs.key_out, s->bufs.val_in, s->bufs.val_out, s->n,
+                               s->sort_end_bit, s->stream));
+    LV_STAGE(2, lvk_bounds_scatter(s->dev, s->bufs, s->stream));
+    LV_STAGE(3, lvk_pair_force(s->dev, s->bufs, s->stream));
+    LV_STAGE(4, lvk_update(s->dev, s->bufs, s->stream));
+#undef LV_STAGE
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s->stream);
+    for (int k = 0; e == cudaSuccess && k < LV_N_STAGES; ++k)
+        e = cudaEventElapsedTime(&ms_out[k], ev[k], ev[k + 1]);
+    for (int k = 0; k <= LV_N_STAGES; ++k) cudaEventDestroy(ev[k]);
+    if (e != cudaSuccess) rc = cuda_fail(s, e, "lv_step_profiled");
+    return rc;
+}
+
+int lv_measure_fp32_peak(void *cuda_stream, double *tflops)
+{
+    if (!tflops) return LV_E_ARG;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return LV_E_CUDA;
+    if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return LV_E_CUDA;
+    float *scratch = nullptr;
+    if (cudaMalloc(&scratch, 256) != cudaSuccess) return LV_E_CUDA;   // measurement aid only
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0);
+    cudaEventCreate(&e1);
+    double best = 0.0, flops = 0.0;
+    cudaError_t e = cudaSuccess;
+    for (int rep = 0; rep < 4 && e == cudaSuccess; ++rep) {
+        cudaEventRecord(e0, st);
+        e = lvk_fma_peak(scratch, sms * 8, 4096, &flops, st);
+        cudaEventRecord(e1, st);
+        if (e == cudaSuccess) e = cudaEventSynchronize(e1);
+        float ms = 0.f;
+        if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, e0, e1);
+        if (e == cudaSuccess && rep > 0 && ms > 0.f) best = std::fmax(best, flops / (ms * 1e-3) * 1e-12);
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    cudaFree(scratch);
+    if (e != cudaSuccess) return LV_E_CUDA;
+    *tflops = best;
+    return LV_OK;
+}
+
+int lv_destroy(lv_sim *s)
+{
+    if (!s) return LV_OK;
+    if (s->bound) cudaStreamSynchronize(s->stream);
+    if (s->graph_exec) cudaGraphExecDestroy(s->graph_exec);
+    if (s->graph) cudaGraphDestroy(s->graph);
+    delete s;
+    return LV_OK;
+}
+
+const char *lv_strerror(int code)
+{
+    switch (code) {
+    case LV_OK: return "ok";
+    case LV_E_ARG: return "bad argument";
+    case LV_E_ORDER: return "call order violated";
+    case LV_E_WORKSPACE: return "workspace too small or misaligned";
+    case LV_E_CUDA: return "CUDA runtime error";
+    case LV_E_NONFINITE: return "non-finite position or velocity";
+    case LV_E_NOMEM: return "host allocation failed";
+    default: return "unknown error";
+    }
+}
+
+const char *lv_last_cuda_error(const lv_sim *s) { return s ? s->cuda_err : ""; }
+
+const char *lv_version(void) { return "lv 0.1.0 (sm_100a)"; }
+
+}  // extern "C"

@@ -1,0 +1,101 @@
+// lv_internal.cuh -- private to csrc/: device parameter block, buffer table and
+// the launch wrappers shared by lv_api.cu, lv_kernels.cu and lv_sort.cu.
+// Nothing here is seen by the oracle (oracle/ shares no code with this tree).
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "lv.h"
+
+// {r_c^2, 48 eps sigma^12, 24 eps sigma^6, k_C q_a q_b} of one type pair, fp32,
+// rounded once from fp64 (include/lv.h: lv_set_types).
+struct LvPair {
+    float rc2, c12, c6, qq;
+};
+
+struct LvTypeDev {
+    float dt_over_m;  // dt / m_a
+    float a, b;       // velocity retention and kick std (R11, R15)
+    float mass;
+    float radius;     // r_a = sigma_a / 2
+    float pad0, pad1, pad2;
+};
+
+struct LvGridDev {
+    float lo, inv_h;
+    int32_t G;
+    uint32_t base;
+};
+
+// Passed BY VALUE to every kernel (__grid_constant__): lives in the constant
+// bank of the launch, so several lv_sim handles never share mutable state.
+struct LvDev {
+    int32_t n, n_types;
+    uint32_t n_cells;
+    int32_t wall_mode;
+    LvPair pair[LV_MAX_TYPES * LV_MAX_TYPES];
+    LvTypeDev type[LV_MAX_TYPES];
+    LvGridDev grid[LV_MAX_TYPES];
+    int8_t w[LV_MAX_TYPES * LV_MAX_TYPES];
+    float dt, g;
+    float om2[3];
+    int32_t sched_mode;
+    int64_t sched_steps;
+    double R0, R1;
+    double wall_k_d[LV_MAX_TYPES];
+    double radius_d[LV_MAX_TYPES];
+    uint32_t seed_lo, seed_hi;
+};
+
+// Device-resident scalars.
+struct LvDevState {
+    long long step;        // index of the next step to take
+    unsigned int status;   // LV_ST_* bits, sticky
+    unsigned int ticket;   // blocks of k_update that have read `step`
+};
+
+struct LvBufs {
+    float4 *posA, *velA;   // current state, slot order of the last rebuild (w: type / id bits)
+    float4 *posB, *velB;   // cell-sorted copy of the current step
+    float4 *force;         // pair force per sorted slot (w: in-range count bits)
+    uint32_t *key_in, *key_out, *val_in, *val_out;
+    uint32_t *cell_off;    // [n_cells + 1]
+    void *sort_temp;
+    size_t sort_temp_bytes;
+    LvDevState *st;
+    unsigned char *staging;  // n * 28 bytes: host<->device state transfers
+};
+
+// droplet radius after n steps (step (iii)); fp64 on host and device
+__host__ __device__ inline double lv_radius_of(int mode, double R0, double R1, long long S, long long n)
+{
+    if (mode == LV_SCHED_CONST || S <= 0) return R0;
+    long long m = n < 0 ? 0 : (n > S ? S : n);
+    if (m == S) return R1;
+    double f = (double)m / (double)S;
+    if (mode == LV_SCHED_LINEAR) return R0 + (R1 - R0) * f;
+    return sqrt(R0 * R0 + (R1 * R1 - R0 * R0) * f);
+}
+
+// ---- launch wrappers (lv_kernels.cu) -- all asynchronous on `st` ----------
+cudaError_t lvk_hash(const LvDev &P, const LvBufs &B, cudaStream_t st);
+cudaError_t lvk_bounds_scatter(const LvDev &P, const LvBufs &B, cudaStream_t st);
+cudaError_t lvk_pair_force(const LvDev &P, const LvBufs &B, cudaStream_t st);
+cudaError_t lvk_update(const LvDev &P, const LvBufs &B, cudaStream_t st);
+cudaError_t lvk_pack_state(const LvDev &P, const LvBufs &B, const float *pos, const float *vel,
+                           const int32_t *type, long long step, cudaStream_t st);
+cudaError_t lvk_unpack_state(const LvDev &P, const LvBufs &B, float *pos, float *vel,
+                             int32_t *type, cudaStream_t st);
+cudaError_t lvk_unpack_forces(const LvDev &P, const LvBufs &B, float *force, int32_t *count,
+                              cudaStream_t st);
+cudaError_t lvk_ids_sorted(const LvDev &P, const LvBufs &B, uint32_t *ids, cudaStream_t st);
+
+// ---- sort (lv_sort.cu): stable LSD radix sort of (key, val) over end_bit bits
+size_t lvs_temp_bytes(int n, int end_bit);
+cudaError_t lvs_sort_pairs(void *temp, size_t temp_bytes, const uint32_t *key_in, uint32_t *key_out,
+                           const uint32_t *val_in, uint32_t *val_out, int n, int end_bit,
+                           cudaStream_t st);
+
+// FP32 FMA throughput probe (lv_measure_fp32_peak)
+cudaError_t lvk_fma_peak(float *scratch, int blocks, int iters, double *flops, cudaStream_t st);

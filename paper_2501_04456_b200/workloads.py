@@ -197,10 +197,14 @@ def fcc_ball(rng, n, sigma, R, jitter=0.05):
     return pts
 
 
-def make_workload(name: str, n: Optional[int] = None, state: bool = True) -> Workload:
+def make_workload(name: str, n: Optional[int] = None, state: bool = True,
+                  seed: Optional[int] = None) -> Workload:
     """BASELINE config `name` ("C1".."C5").  With n given, a scaled-down (or
-    up) copy at the same volume fractions: radii scale as (n/N)^(1/3)."""
+    up) copy at the same volume fractions: radii scale as (n/N)^(1/3).  `seed`
+    overrides the configuration's seed (independent replicas)."""
     w = _spec(name)
+    if seed is not None:
+        w = replace(w, seed=int(seed))
     if n is not None and n != w.n:
         f = (n / w.n) ** (1.0 / 3.0)
         w = replace(w, n=n, R0=w.R0 * f, R1=w.R1 * f, name=f"{w.name}@{n}")

@@ -1,0 +1,360 @@
+"""Parity of the CUDA path (through the C ABI, include/lv.h) with the fp64 CPU
+oracle on the same seeded inputs.  Bars (BASELINE.json north_star; DESIGN.md
+"Parity protocol"): cell keys, sort permutation, cell offsets and neighbour
+counts BIT-EXACT; forces max_i |dF_i|_inf / S_i <= 1e-5; one-step velocities
+and positions <= 1e-5 (relative to |v| + sqrt(kT/m), resp. R); 100 steps
+<= 1e-3 R.  All tests need a GPU."""
+import numpy as np
+import pytest
+
+from paper_2501_04456_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+FORCE_TOL = 1e-5
+
+
+@pytest.fixture(scope="module")
+def B():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_2501_04456_b200 import binding
+    binding.load()
+    return binding
+
+
+CASES = [          # (config, n or None for full size, cells_per_cut)
+    ("C1", None, None),
+    ("C1", None, [2]),
+    ("C2", 8192, None),
+    ("C2", 8191, [2, 3]),
+    ("C3", 20000, None),
+    ("C3", 20000, [1, 2, 2]),
+    ("C4", 20000, None),
+    ("C4", 19999, [2]),
+    ("C5", 20001, None),
+]
+
+_cache = {}
+
+
+def workload(name, n):
+    key = (name, n)
+    if key not in _cache:
+        _cache[key] = W.make_workload(name, n)
+    return _cache[key]
+
+
+def force_error(Fg, Fo, So):
+    err = np.abs(Fg.astype(np.float64) - Fo).max(axis=1)
+    zero = So == 0
+    assert np.all(Fg[zero] == 0.0)
+    return (err[~zero] / So[~zero]).max() if (~zero).any() else 0.0
+
+
+@pytest.mark.parametrize("name,n,cpc", CASES)
+def test_cell_structures_bit_exact(B, orc, name, n, cpc):
+    w = workload(name, n)
+    p = orc.params_from_workload(w)
+    g = orc.grid_spec(p, cpc)
+    sim = B.Simulation.from_workload(w, cells_per_cut=cpc)
+    sim.compute_forces()
+    gg = sim.grid()
+    T = w.n_types
+    assert gg.n_types == g.n_types
+    for b in range(T):
+        assert gg.G[b] == g.G[b] and gg.base[b] == g.base[b]
+        assert np.float32(gg.lo[b]).tobytes() == np.float32(g.lo[b]).tobytes()
+        assert np.float32(gg.inv_h[b]).tobytes() == np.float32(g.inv_h[b]).tobytes()
+        assert gg.h[b] == g.h[b]
+        for a in range(T):
+            assert gg.w[a * 8 + b] == g.w[a * 8 + b]
+    assert gg.base[T] == g.base[T]
+    key, ks, perm, off = orc.cell_structures(g, w.pos, w.type)
+    assert np.array_equal(sim.get_debug(B.DBG_KEYS), key)
+    assert np.array_equal(sim.get_debug(B.DBG_KEYS_SORTED), ks)
+    assert np.array_equal(sim.get_debug(B.DBG_PERM), perm)
+    assert np.array_equal(sim.get_debug(B.DBG_CELL_OFFSETS), off)
+    assert np.array_equal(sim.get_debug(B.DBG_IDS_SORTED), perm)   # slot = id after set_state
+    assert sim.status() == 0
+    sim.close()
+
+
+@pytest.mark.parametrize("name,n,cpc", CASES)
+def test_forces_and_counts(B, orc, name, n, cpc):
+    w = workload(name, n)
+    p = orc.params_from_workload(w)
+    Fo, So, co, _ = orc.pair_forces(p, w.pos, w.type, "cells")
+    sim = B.Simulation.from_workload(w, cells_per_cut=cpc)
+    sim.compute_forces()
+    Fg, cg = sim.get_forces()
+    assert np.array_equal(cg, co)                     # neighbour counts bit-exact
+    assert co.sum() > 0
+    assert force_error(Fg, Fo, So) <= FORCE_TOL
+    # Newton III on the GPU result itself
+    assert np.all(np.abs(Fg.astype(np.float64).sum(axis=0)) <= 1e-5 * So.sum())
+    sim.close()
+
+
+@pytest.mark.parametrize("name", ["C3", "C4", "C5"])
+def test_forces_full_size(B, orc, name):
+    """BASELINE sizes (N = 2.5e5, 2^20), the launch configuration bench.py times."""
+    w = workload(name, None)
+    p = orc.params_from_workload(w)
+    Fo, So, co, _ = orc.pair_forces(p, w.pos, w.type, "cells")
+    sim = B.Simulation.from_workload(w)
+    sim.compute_forces()
+    Fg, cg = sim.get_forces()
+    assert np.array_equal(cg, co)
+    assert force_error(Fg, Fo, So) <= FORCE_TOL
+    ks = sim.get_debug(B.DBG_KEYS_SORTED)
+    assert np.all(np.diff(ks.astype(np.int64)) >= 0)
+    assert np.array_equal(np.sort(sim.get_debug(B.DBG_PERM)), np.arange(w.n, dtype=np.uint32))
+    off = sim.get_debug(B.DBG_CELL_OFFSETS)
+    assert off[0] == 0 and off[-1] == w.n and np.all(np.diff(off.astype(np.int64)) >= 0)
+    sim.close()
+
+
+def test_dense_compressed_state(B, orc):
+    """A crowded state (C2 pushed to its final radius): hundreds of NPs per
+    cell, long rows."""
+    w = W.make_workload("C2", 8192)
+    f = 0.55
+    w.pos = (w.pos * np.float32(f)).astype(np.float32)
+    w.R0 *= f
+    w.R1 *= f
+    p = orc.params_from_workload(w)
+    Fo, So, co, _ = orc.pair_forces(p, w.pos, w.type, "cells")
+    sim = B.Simulation.from_workload(w)
+    sim.compute_forces()
+    Fg, cg = sim.get_forces()
+    assert np.array_equal(cg, co) and co.mean() > 150
+    assert force_error(Fg, Fo, So) <= FORCE_TOL
+    sim.close()
+
+
+def vel_pos_check(w, p_orc, xo, vo, xg, vg, S_pair, R):
+    m = np.asarray(w.mass)[w.type]
+    vscale = np.linalg.norm(vo, axis=1) + np.sqrt(w.kT / m)
+    dv = np.abs(vg.astype(np.float64) - vo).max(axis=1)
+    tol_v = 1e-5 * vscale + (w.dt / m) * FORCE_TOL * S_pair
+    assert np.all(dv <= tol_v), float((dv / tol_v).max())
+    dx = np.abs(xg.astype(np.float64) - xo).max(axis=1)
+    assert dx.max() / R <= 1e-5
+
+
+@pytest.mark.parametrize("name,n", [("C1", None), ("C2", 8192), ("C3", 20000), ("C4", 20000), ("C5", 20001)])
+def test_one_step(B, orc, name, n):
+    w = workload(name, n)
+    p = orc.params_from_workload(w)
+    xo, vo, bad = orc.step(p, w.pos, w.vel, w.type, step0=0, nsteps=1)
+    _, So, _, _ = orc.pair_forces(p, w.pos, w.type, "cells")
+    sim = B.Simulation.from_workload(w)
+    sim.step(1)
+    xg, vg, tg, R, st = sim.get_state()
+    assert bad == 0 and st == 1
+    assert np.array_equal(tg, w.type)
+    assert R == pytest.approx(orc.radius(p, 1), rel=1e-15)
+    vel_pos_check(w, p, xo, vo, xg, vg, So, R)
+    sim.close()
+
+
+def test_one_step_late_schedule_and_near_wall(B, orc):
+    """A step taken late in the schedule with many NPs pressed against the
+    moving interface: the surface term dominates and |x| - (R - r) is a
+    cancellation (fp64 sub-expression on the GPU)."""
+    w = W.make_workload("C3", 20000)
+    step0 = 6000
+    R = w.R0 + (w.R1 - w.R0) * step0 / w.sched_steps
+    r = np.linalg.norm(w.pos.astype(np.float64), axis=1, keepdims=True)
+    scale = np.where(r > R - 1.4, (R - 1.4 + 0.5 * np.random.default_rng(0).random(r.shape)) / r, 1.0)
+    w.pos = (w.pos * scale).astype(np.float32)
+    p = orc.params_from_workload(w)
+    xo, vo, bad, Fp, Fe = orc.step(p, w.pos, w.vel, w.type, step0=step0, nsteps=1, want_forces=True)
+    assert (np.abs(Fe).max(axis=1) > 1.0).sum() > 500        # the wall is really felt
+    _, So, _, _ = orc.pair_forces(p, w.pos, w.type, "cells")
+    Sw = np.abs(Fe).sum(axis=1)
+    sim = B.Simulation.from_workload(w, load_state=False)
+    sim.set_state(w.pos, w.vel, w.type, step0)
+    sim.step(1)
+    xg, vg, _, Rg, st = sim.get_state()
+    assert st == step0 + 1 and Rg == pytest.approx(orc.radius(p, step0 + 1), rel=1e-15)
+    vel_pos_check(w, p, xo, vo, xg, vg, So + Sw, Rg)
+    sim.close()
+
+
+@pytest.mark.parametrize("name,n", [("C1", None), ("C2", 8192), ("C4", 8000)])
+def test_hundred_steps(B, orc, name, n):
+    w = workload(name, n)
+    p = orc.params_from_workload(w)
+    xo, vo, bad = orc.step(p, w.pos, w.vel, w.type, step0=0, nsteps=100)
+    sim = B.Simulation.from_workload(w)
+    sim.step(100)
+    xg, vg, _, R, st = sim.get_state()
+    assert bad == 0 and st == 100
+    assert R == pytest.approx(orc.radius(p, 100), rel=1e-15)
+    d = np.linalg.norm(xg.astype(np.float64) - xo, axis=1)
+    assert d.max() <= 1e-3 * R, d.max() / R
+    sim.close()
+
+
+def test_noise_matches_oracle_draws(B, orc):
+    """a = 0, no forces, v0 = 0  ->  v1 = b xi: the GPU's Philox/Box-Muller
+    draws against the oracle's, particle by particle, at a 64-bit step index."""
+    n, b, seed, step0 = 5000, 0.75, 0xDEADBEEF12345678, (3 << 32) + 17
+    sim = B.Simulation(n, 1, seed, 0.01)
+    sim.set_types([dict(sigma=1.0, eps=0.0, mass=1.0, drag_a=0.0, kick_b=b)], cut_factor=40.0)
+    sim.set_droplet_schedule(B.SCHED_CONST, 500.0)
+    sim.bind()
+    g = np.arange(18) * 50.0 - 425.0
+    x0 = np.stack(np.meshgrid(g, g, g, indexing="ij"), -1).reshape(-1, 3)[:n].astype(np.float32)
+    sim.set_state(x0, np.zeros((n, 3), np.float32), np.zeros(n, np.int32), step0)
+    sim.step(1)
+    _, v, _, _, st = sim.get_state()
+    xi = orc.gauss3(seed, np.arange(n), step0)
+    assert st == step0 + 1
+    assert np.abs(v / b - xi).max() < 2e-6
+    sim.close()
+
+
+def test_split_invariance_and_roundtrip(B):
+    w = workload("C2", 8192)
+    s1 = B.Simulation.from_workload(w)
+    s1.step(30)
+    a = s1.get_state()
+    s2 = B.Simulation.from_workload(w)
+    s2.step(12)
+    s2.step(18)
+    b = s2.get_state()
+    for u, v in zip(a[:3], b[:3]):
+        assert np.array_equal(u, v)
+    assert a[3:] == b[3:]
+    # get -> set -> get is the identity (restart path)
+    s3 = B.Simulation.from_workload(w, load_state=False)
+    s3.set_state(a[0], a[1], a[2], a[4])
+    c = s3.get_state()
+    for u, v in zip(a[:3], c[:3]):
+        assert np.array_equal(u, v)
+    assert c[4] == 30
+    # device-buffer variant of the accessors
+    import torch
+    pd, vd, td, R, st = s1.get_state(on_device=True)
+    torch.cuda.synchronize()
+    assert np.array_equal(pd.cpu().numpy(), a[0]) and np.array_equal(td.cpu().numpy(), a[2])
+    s3.set_state(pd, vd, td, 30)
+    c = s3.get_state()
+    assert np.array_equal(c[0], a[0]) and np.array_equal(c[1], a[1])
+    for s in (s1, s2, s3):
+        s.close()
+
+
+def test_restart_continues_within_tolerance(B):
+    """Stop, save, restart: same noise (keyed on id and step);
+    only the summation order changes, so the continuation agrees to rounding."""
+    w = workload("C1", None)
+    s1 = B.Simulation.from_workload(w)
+    s1.step(20)
+    mid = s1.get_state()
+    s1.step(20)
+    end = s1.get_state()
+    s2 = B.Simulation.from_workload(w, load_state=False)
+    s2.set_state(mid[0], mid[1], mid[2], mid[4])
+    s2.step(20)
+    end2 = s2.get_state()
+    assert end2[4] == 40
+    assert np.abs(end2[0] - end[0]).max() < 1e-4
+    s1.close()
+    s2.close()
+
+
+@pytest.mark.parametrize("n", [0, 1, 2, 33, 129])
+def test_tiny_and_empty(B, orc, n):
+    rng = np.random.default_rng(n)
+    x = (rng.uniform(-1.5, 1.5, size=(n, 3))).astype(np.float32)
+    if n >= 2:
+        g = np.arange(6) * 1.1 - 2.75
+        x = np.stack(np.meshgrid(g, g, g, indexing="ij"), -1).reshape(-1, 3)[:n].astype(np.float32)
+    v = rng.normal(0, 1, size=(n, 3)).astype(np.float32)
+    t = np.zeros(n, np.int32)
+    a, b = orc.langevin_coeffs(1.0, 1.0, 1.0, 0.005)
+    p = orc.make_params(sigma=[1.0], mass=[1.0], charge=[0.0], wall_k=[100.0], drag_a=[a], kick_b=[b],
+                        dt=0.005, eps=[1.0], cut_factor=2.5, R0=6.0, seed=5)
+    sim = B.Simulation(n, 1, 5, 0.005)
+    ga, gb = B.langevin_coeffs(1.0, 1.0, 1.0, 0.005)
+    sim.set_types([dict(sigma=1.0, eps=1.0, mass=1.0, wall_k=100.0, drag_a=ga, kick_b=gb)], cut_factor=2.5)
+    sim.set_droplet_schedule(B.SCHED_CONST, 6.0)
+    sim.bind()
+    sim.set_state(x, v, t, 0)
+    sim.compute_forces()
+    Fg, cg = sim.get_forces()
+    Fo, So, co, _ = orc.pair_forces(p, x, t, "brute")
+    assert np.array_equal(cg, co)
+    if n:
+        assert force_error(Fg, Fo, So) <= FORCE_TOL
+    sim.step(3)
+    xg, vg, tg, R, st = sim.get_state()
+    xo, vo, _ = orc.step(p, x, v, t, nsteps=3, method="brute")
+    assert st == (3 if n else 0) or n == 0
+    if n:
+        assert np.abs(xg - xo).max() < 1e-4 and np.abs(vg - vo).max() < 1e-3
+    sim.close()
+
+
+def test_status_flags(B):
+    w = workload("C1", None)
+    sim = B.Simulation.from_workload(w, load_state=False)
+    pos = w.pos.copy()
+    pos[7] = pos[8]                       # coincident pair: no core clamp (R6)
+    sim.set_state(pos, w.vel, w.type, 0)
+    sim.step(1)
+    with pytest.raises(B.LvError) as e:
+        sim.get_state()
+    assert e.value.code == B.E_NONFINITE
+    assert sim.status() & B.ST_NONFINITE
+    # set_state clears the sticky bit
+    sim.set_state(w.pos, w.vel, w.type, 0)
+    sim.step(1)
+    sim.get_state()
+    assert sim.status() == 0
+    # NaN injected
+    pos = w.pos.copy()
+    pos[100, 1] = np.nan
+    sim.set_state(pos, w.vel, w.type, 0)
+    sim.step(1)
+    assert sim.status() & B.ST_NONFINITE
+    # far outside the grid: warning only, forces still right for the others
+    pos = w.pos.copy()
+    pos[5] = [500.0, 0.0, 0.0]
+    sim.set_state(pos, w.vel, w.type, 0)
+    sim.compute_forces()
+    assert sim.status() == B.ST_OUTSIDE_GRID
+    sim.close()
+
+
+def test_wall_window_mode_and_r2law(B, orc):
+    w = W.make_workload("C1", None)
+    w.wall_mode = W.WALL_WINDOW
+    w.sched_mode, w.R1, w.sched_steps = W.SCHED_R2LAW, 12.0, 50
+    p = orc.params_from_workload(w)
+    xo, vo, bad = orc.step(p, w.pos, w.vel, w.type, step0=0, nsteps=40)
+    sim = B.Simulation.from_workload(w)
+    sim.step(40)
+    xg, vg, _, R, st = sim.get_state()
+    assert R == pytest.approx(orc.radius(p, 40), rel=1e-14)
+    d = np.linalg.norm(xg.astype(np.float64) - xo, axis=1)
+    assert d.max() <= 1e-3 * R
+    sim.close()
+
+
+def test_explicit_interaction_matrix(B, orc):
+    """PAPER.md:82 (Table 1, two-size run): a non-Berthelot eps matrix."""
+    w = W.make_workload("C2", 8192)
+    w.eps_matrix = 0.23 * np.array([[0.155, 1.26], [1.26, 0.155]])
+    p = orc.params_from_workload(w)
+    Fo, So, co, _ = orc.pair_forces(p, w.pos, w.type, "cells")
+    sim = B.Simulation.from_workload(w)
+    sim.compute_forces()
+    Fg, cg = sim.get_forces()
+    assert np.array_equal(cg, co)
+    assert force_error(Fg, Fo, So) <= FORCE_TOL
+    sim.close()
