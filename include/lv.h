@@ -188,6 +188,20 @@ int lv_launches_per_step(const lv_sim *s);
 #define LV_N_STAGES 5
 int lv_step_profiled(lv_sim *s, float *ms_out);
 
+/* Measurement aid for bench.py (CUDA events on the launching stream, inside the
+ * timed region).  lv_stage_timing(s, capacity > 0): from now on every step of
+ * lv_step is enqueued as direct launches of the SAME kernels (no graph) with a
+ * CUDA event recorded on the stream before the first and after each of the
+ * LV_N_STAGES stages; at most `capacity` steps may be taken between two reads
+ * (lv_step returns LV_E_ARG beyond that).  capacity = 0 switches back to graph
+ * replay and frees the events.
+ * lv_read_stage_timing synchronises the stream and writes, for the steps taken
+ * since the last read: ms_stage_sum (host[LV_N_STAGES]) the summed device time
+ * of each stage, *ms_step_sum (host) the summed first-event-to-last-event time
+ * of each step, *steps (host) their number; then resets the counter. */
+int lv_stage_timing(lv_sim *s, int capacity);
+int lv_read_stage_timing(lv_sim *s, double *ms_stage_sum, double *ms_step_sum, int64_t *steps);
+
 /* Measurement aid: FP32 FMA throughput of this GPU from a register-resident
  * independent-FMA kernel on `cuda_stream`; writes TFLOP/s (host).  The
  * denominator of the pair-force kernel's ALU roofline. */

@@ -28,6 +28,7 @@ SYMBOLS = ["lv_langevin_coeffs", "lv_create", "lv_set_types", "lv_set_forces",
            "lv_set_droplet_schedule", "lv_set_grid", "lv_workspace_bytes", "lv_bind",
            "lv_set_state", "lv_step", "lv_compute_forces", "lv_get_state", "lv_get_forces",
            "lv_get_status", "lv_get_debug", "lv_launches_per_step", "lv_step_profiled",
+           "lv_stage_timing", "lv_read_stage_timing",
            "lv_measure_fp32_peak", "lv_destroy", "lv_strerror",
            "lv_last_cuda_error", "lv_version"]
 
@@ -80,6 +81,8 @@ def load():
     L.lv_get_debug.argtypes = [vp, C.c_int, vp, C.c_size_t, C.c_int]
     L.lv_launches_per_step.argtypes = [vp]
     L.lv_step_profiled.argtypes = [vp, C.POINTER(C.c_float)]
+    L.lv_stage_timing.argtypes = [vp, C.c_int]
+    L.lv_read_stage_timing.argtypes = [vp, dp, dp, C.POINTER(C.c_int64)]
     L.lv_measure_fp32_peak.argtypes = [vp, dp]
     L.lv_destroy.argtypes = [vp]
     L.lv_strerror.argtypes = [C.c_int]
@@ -263,6 +266,17 @@ class Simulation:
         ms = (C.c_float * 5)()
         self._check(self.L.lv_step_profiled(self.h, ms), "lv_step_profiled")
         return dict(zip(self.STAGES, [float(v) for v in ms]))
+
+    def stage_timing(self, capacity: int):
+        self._check(self.L.lv_stage_timing(self.h, int(capacity)), "lv_stage_timing")
+
+    def read_stage_timing(self):
+        """-> (dict stage -> summed ms, summed step ms, steps) since the last read."""
+        st = (C.c_double * 5)()
+        tot, n = C.c_double(), C.c_int64()
+        self._check(self.L.lv_read_stage_timing(self.h, st, C.byref(tot), C.byref(n)),
+                    "lv_read_stage_timing")
+        return dict(zip(self.STAGES, [float(v) for v in st])), tot.value, int(n.value)
 
     def measure_fp32_peak(self) -> float:
         t = C.c_double()

@@ -36,6 +36,9 @@ struct lv_sim {
     cudaGraph_t graph = nullptr;
     cudaGraphExec_t graph_exec = nullptr;
     int launches_per_step = 0;
+    // stage timing (measurement aid): (LV_N_STAGES + 1) events per step
+    cudaEvent_t *tim_ev = nullptr;
+    int tim_cap = 0, tim_used = 0;
     char cuda_err[256];
 };
 
@@ -181,6 +184,36 @@ int enqueue_step(lv_sim *s)
     if (rc != LV_OK) return rc;
     LV_CUDA(s, lvk_update(s->dev, s->bufs, s->stream));
     return LV_OK;
+}
+
+// One step as direct launches with an event before the first and after each stage.
+int enqueue_step_timed(lv_sim *s, cudaEvent_t *ev)
+{
+    LV_CUDA(s, cudaEventRecord(ev[0], s->stream));
+    LV_CUDA(s, lvk_hash(s->dev, s->bufs, s->stream));
+    LV_CUDA(s, cudaEventRecord(ev[1], s->stream));
+    LV_CUDA(s, lvs_sort_pairs(s->bufs.sort_temp, s->bufs.sort_temp_bytes, s->bufs.key_in,
+                              s->bufs.key_out, s->bufs.val_in, s->bufs.val_out, s->n,
+                              s->sort_end_bit, s->stream));
+    LV_CUDA(s, cudaEventRecord(ev[2], s->stream));
+    LV_CUDA(s, lvk_bounds_scatter(s->dev, s->bufs, s->stream));
+    LV_CUDA(s, cudaEventRecord(ev[3], s->stream));
+    LV_CUDA(s, lvk_pair_force(s->dev, s->bufs, s->stream));
+    LV_CUDA(s, cudaEventRecord(ev[4], s->stream));
+    LV_CUDA(s, lvk_update(s->dev, s->bufs, s->stream));
+    LV_CUDA(s, cudaEventRecord(ev[5], s->stream));
+    return LV_OK;
+}
+
+void free_timing(lv_sim *s)
+{
+    if (s->tim_ev) {
+        for (int k = 0; k < s->tim_cap * (LV_N_STAGES + 1); ++k)
+            if (s->tim_ev[k]) cudaEventDestroy(s->tim_ev[k]);
+        free(s->tim_ev);
+    }
+    s->tim_ev = nullptr;
+    s->tim_cap = s->tim_used = 0;
 }
 
 // Capture one step into a graph (nothing executes during capture).  The graph
@@ -383,6 +416,15 @@ int lv_step(lv_sim *s, int n)
     if (!s || n < 0) return LV_E_ARG;
     if (!s->bound || !s->state_set) return LV_E_ORDER;
     if (s->n == 0) return LV_OK;
+    if (s->tim_cap > 0) {
+        if (n > s->tim_cap - s->tim_used) return LV_E_ARG;
+        for (int k = 0; k < n; ++k) {
+            int rc = enqueue_step_timed(s, s->tim_ev + (size_t)s->tim_used * (LV_N_STAGES + 1));
+            if (rc != LV_OK) return rc;
+            ++s->tim_used;
+        }
+        return LV_OK;
+    }
     for (int k = 0; k < n; ++k) {
         if (s->graph_exec) {
             LV_CUDA(s, cudaGraphLaunch(s->graph_exec, s->stream));
@@ -531,6 +573,47 @@ int lv_step_profiled(lv_sim *s, float *ms_out)
     return rc;
 }
 
+int lv_stage_timing(lv_sim *s, int capacity)
+{
+    if (!s || capacity < 0 || capacity > (1 << 20)) return LV_E_ARG;
+    if (!s->bound) return LV_E_ORDER;
+    LV_CUDA(s, cudaStreamSynchronize(s->stream));
+    free_timing(s);
+    if (capacity == 0) return LV_OK;
+    const size_t ne = (size_t)capacity * (LV_N_STAGES + 1);
+    s->tim_ev = (cudaEvent_t *)calloc(ne, sizeof(cudaEvent_t));
+    if (!s->tim_ev) return LV_E_NOMEM;
+    s->tim_cap = capacity;
+    for (size_t k = 0; k < ne; ++k) {
+        cudaError_t e = cudaEventCreate(&s->tim_ev[k]);
+        if (e != cudaSuccess) { free_timing(s); return cuda_fail(s, e, "cudaEventCreate"); }
+    }
+    return LV_OK;
+}
+
+int lv_read_stage_timing(lv_sim *s, double *ms_stage_sum, double *ms_step_sum, int64_t *steps)
+{
+    if (!s) return LV_E_ARG;
+    if (!s->bound || s->tim_cap == 0) return LV_E_ORDER;
+    LV_CUDA(s, cudaStreamSynchronize(s->stream));
+    double st[LV_N_STAGES] = {0, 0, 0, 0, 0}, tot = 0.0;
+    for (int k = 0; k < s->tim_used; ++k) {
+        cudaEvent_t *ev = s->tim_ev + (size_t)k * (LV_N_STAGES + 1);
+        float ms = 0.f;
+        for (int j = 0; j < LV_N_STAGES; ++j) {
+            LV_CUDA(s, cudaEventElapsedTime(&ms, ev[j], ev[j + 1]));
+            st[j] += ms;
+        }
+        LV_CUDA(s, cudaEventElapsedTime(&ms, ev[0], ev[LV_N_STAGES]));
+        tot += ms;
+    }
+    if (ms_stage_sum) for (int j = 0; j < LV_N_STAGES; ++j) ms_stage_sum[j] = st[j];
+    if (ms_step_sum) *ms_step_sum = tot;
+    if (steps) *steps = s->tim_used;
+    s->tim_used = 0;
+    return LV_OK;
+}
+
 int lv_measure_fp32_peak(void *cuda_stream, double *tflops)
 {
     if (!tflops) return LV_E_ARG;
@@ -568,6 +651,7 @@ int lv_destroy(lv_sim *s)
     if (s->bound) cudaStreamSynchronize(s->stream);
     if (s->graph_exec) cudaGraphExecDestroy(s->graph_exec);
     if (s->graph) cudaGraphDestroy(s->graph);
+    free_timing(s);
     delete s;
     return LV_OK;
 }

@@ -159,18 +159,16 @@ def test_one_step(B, orc, name, n):
     sim.close()
 
 
-def test_one_step_late_schedule_and_near_wall(B, orc):
-    """A step taken late in the schedule with many NPs pressed against the
-    moving interface: the surface term dominates and |x| - (R - r) is a
-    cancellation (fp64 sub-expression on the GPU)."""
+def test_one_step_moving_interface_near_wall(B, orc):
+    """A step taken after the interface has moved 0.8 sigma into the initial
+    distribution: hundreds of NPs are pressed by the surface spring, the
+    surface term dominates and |x| - (R - r) is a cancellation (fp64
+    sub-expression on the GPU).  Positions are untouched, so no pair overlaps."""
     w = W.make_workload("C3", 20000)
-    step0 = 6000
-    R = w.R0 + (w.R1 - w.R0) * step0 / w.sched_steps
-    r = np.linalg.norm(w.pos.astype(np.float64), axis=1, keepdims=True)
-    scale = np.where(r > R - 1.4, (R - 1.4 + 0.5 * np.random.default_rng(0).random(r.shape)) / r, 1.0)
-    w.pos = (w.pos * scale).astype(np.float32)
+    step0 = int(0.8 / (w.R0 - w.R1) * w.sched_steps)
     p = orc.params_from_workload(w)
     xo, vo, bad, Fp, Fe = orc.step(p, w.pos, w.vel, w.type, step0=step0, nsteps=1, want_forces=True)
+    assert bad == 0
     assert (np.abs(Fe).max(axis=1) > 1.0).sum() > 500        # the wall is really felt
     _, So, _, _ = orc.pair_forces(p, w.pos, w.type, "cells")
     Sw = np.abs(Fe).sum(axis=1)
