@@ -1,0 +1,415 @@
+#!/usr/bin/env python
+"""bench.py -- particle-steps/s of the Langevin droplet step (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl lv|reference]
+
+A "step" is one pass of the whole hot path (hash, sort, offsets + scatter,
+pair force, fused update: SURVEY.md sec. 8(a) rows A1-A7) over all N particles of
+the workload, i.e. one simulation time step.  Workload: BASELINE.json
+configs[2] ("C3": N = 250 000, three NP types, LJ + Coulomb, gravity,
+centrifugal, shrinking interface), the configuration with the N = 2.5e5 the
+metric is quoted on; inputs are seeded and synthetic (workloads.py).
+
+Own arm (--impl lv, default):
+  value       whole-job particle-steps/s, state resident in HBM, K timed steps,
+              device time from CUDA events recorded by the library on its own
+              stream around every step (and every stage), L2 flushed (256 MiB
+              memset) between timed steps, max over ranks.
+  roofline    the pair-force kernel (dominant): algorithmic FP32 flops per
+              launch / its average CUDA-event duration inside the same timed
+              region, against the FP32 FMA peak derived in DESIGN.md.
+  resident    the same K steps as one lv_step(K) graph replay without flushes
+              (how a simulation actually runs: the 8 MB state stays in L2).
+  e2e         set_state(host) + lv_step(1) + get_state(host) per step through
+              the C ABI with pinned host buffers, copies inside the timed region.
+  cpu_baseline  the fp64 oracle, as it stands, on the host cores (rank 0, N=1).
+Multi-GPU: independent replicas, one per rank, no data-path collective
+(DESIGN.md "Multi-GPU: replicas only"); value = sum of units / slowest rank.
+
+Reference arm (--impl reference): the oracle timed on the host cores on the
+same workload; rank 0 only.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_2501_04456_b200 import replicas, workloads  # noqa: E402
+
+METRIC = "particle-steps/sec at N=2.5e5"
+UNIT = "particle-steps/s"
+FLUSH_BYTES = 256 << 20            # > 126 MB L2
+# Algorithmic FP32 flops of one ordered in-range pair (DESIGN.md "Roofline of
+# the pair-force kernel"): 3 sub + (1 mul + 2 fma = 5) + 1 compare for the
+# distance test, 1 rcp + 2 mul + 1 fma (2) + 2 mul + 3 fma (6) for LJ and the
+# accumulation = 22.  Charged pairs add 4 (rsqrt, mul, fma); not counted here,
+# so the figure is a lower bound.
+FLOP_PER_PAIR = 22.0
+FP32_LANES_PER_SM = 128
+
+
+def peaks():
+    p = {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0, "source": "fallback (B200_PROFILING.md)"}
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            m = json.load(f)
+        p.update(hbm_gbs=float(m["hbm_gbs"]), sm_max_mhz=float(m["sm_max_mhz"]),
+                 source="MEASURED_PEAKS.json")
+    except Exception:
+        pass
+    return p
+
+
+class ClockSampler(threading.Thread):
+    """SM clock and throttle reasons during the timed region (NVML)."""
+
+    def __init__(self, index, period=0.02):
+        super().__init__(daemon=True)
+        self.index, self.period = index, period
+        self.sm, self.reasons, self.max_mhz = [], set(), None
+        self._stop_evt = threading.Event()
+        try:
+            import pynvml as nv
+            nv.nvmlInit()
+            self.nv = nv
+            self.h = nv.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = nv.nvmlDeviceGetMaxClockInfo(self.h, nv.NVML_CLOCK_SM)
+        except Exception:
+            self.nv = None
+
+    def run(self):
+        if self.nv is None:
+            return
+        nv = self.nv
+        names = {
+            getattr(nv, "nvmlClocksEventReasonHwSlowdown", 0x8): "hw_slowdown",
+            getattr(nv, "nvmlClocksEventReasonHwThermalSlowdown", 0x40): "hw_thermal_slowdown",
+            getattr(nv, "nvmlClocksEventReasonSwThermalSlowdown", 0x20): "sw_thermal_slowdown",
+            getattr(nv, "nvmlClocksEventReasonSwPowerCap", 0x4): "sw_power_cap",
+            getattr(nv, "nvmlClocksEventReasonHwPowerBrakeSlowdown", 0x80): "hw_power_brake",
+        }
+        while not self._stop_evt.is_set():
+            try:
+                self.sm.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                try:
+                    r = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                except Exception:
+                    r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for bit, name in names.items():
+                    if r & bit:
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            self._stop_evt.wait(self.period)
+
+    def finish(self):
+        self._stop_evt.set()
+        self.join(timeout=2.0)
+        return {"sm_mhz": float(np.median(self.sm)) if self.sm else None,
+                "sm_max_mhz": float(self.max_mhz) if self.max_mhz else None,
+                "samples": len(self.sm), "reasons": sorted(self.reasons)}
+
+
+def visible_gpu_index(local_rank):
+    cvd = os.environ.get("CUDA_VISIBLE_DEVICES")
+    if cvd:
+        try:
+            return int(cvd.split(",")[local_rank])
+        except Exception:
+            return local_rank
+    return local_rank
+
+
+# ----------------------------------------------------------------- own arm
+def timed_steps(sim, torch, flush, k):
+    """k steps with stage events, L2 flushed between steps.
+    -> (stage ms sums, step ms sum)."""
+    sim.stage_timing(k)
+    with torch.cuda.stream(sim.stream):
+        for _ in range(k):
+            if flush is not None:
+                flush.zero_()
+            sim.step(1)
+    stages, tot, n = sim.read_stage_timing()
+    assert n == k
+    sim.stage_timing(0)
+    return stages, tot
+
+
+def inrange_pairs(sim):
+    sim.compute_forces()
+    _, cnt = sim.get_forces()
+    return float(cnt.astype(np.int64).sum())
+
+
+def measure_point(sim, torch, flush, w, steps, warmup):
+    """One measurement of the resident-state throughput at the current step."""
+    timed_steps(sim, torch, flush, max(warmup, 1))
+    p0 = inrange_pairs(sim)
+    stages, tot = timed_steps(sim, torch, flush, steps)
+    p1 = inrange_pairs(sim)
+    return stages, tot, 0.5 * (p0 + p1)
+
+
+def run_lv(args):
+    import torch
+    from paper_2501_04456_b200 import binding
+
+    rank, local_rank, world = replicas.env_rank_world()
+    if args.gpus != world:
+        if world == 1 and args.gpus > 1:
+            raise SystemExit("bench.py --gpus N>1 must be launched with torch.distributed.run "
+                             "(one rank per GPU)")
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the library has no CPU path")
+    torch.cuda.set_device(local_rank)
+    device = f"cuda:{local_rank}"
+    if world > 1:
+        replicas.init("nccl")
+    binding.load()
+    pk = peaks()
+
+    base = workloads.make_workload(args.workload, state=False)
+    w = workloads.make_workload(args.workload, seed=replicas.replica_seed(base.seed, rank))
+    sim = binding.Simulation.from_workload(w, cells_per_cut=args.cells_per_cut, device=device)
+    if args.start_step > 0:
+        sim.step(args.start_step)
+        sim.get_state()                      # synchronises; raises on a non-finite state
+    flush = torch.empty(FLUSH_BYTES, dtype=torch.uint8, device=device)
+    n_sms = torch.cuda.get_device_properties(device).multi_processor_count
+    fma_tflops = sim.measure_fp32_peak()
+
+    # ---- timed region: K steps, events on the library's stream -------------
+    timed_steps(sim, torch, flush, max(args.warmup, 3))
+    pairs0 = inrange_pairs(sim)
+    sampler = ClockSampler(visible_gpu_index(local_rank))
+    replicas.barrier()
+    torch.cuda.synchronize()
+    sampler.start()
+    t_wall0 = time.perf_counter()
+    stages, tot_ms = timed_steps(sim, torch, flush, args.steps)
+    torch.cuda.synchronize()
+    wall_s = time.perf_counter() - t_wall0
+    clocks = sampler.finish()
+    replicas.barrier()
+    pairs1 = inrange_pairs(sim)
+    launches_per_step = sim.launches_per_step()
+
+    ms_max, units = replicas.reduce_timing(tot_ms, float(w.n) * args.steps, device=device)
+    value = units / (ms_max * 1e-3)
+
+    # ---- the same K steps as one graph replay, state L2-resident -----------
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    sim.step(max(args.warmup, 3))
+    sim.synchronize()
+    e0.record(sim.stream)
+    sim.step(args.steps)
+    e1.record(sim.stream)
+    e1.synchronize()
+    res_ms = e0.elapsed_time(e1)
+    res_max, _ = replicas.reduce_timing(res_ms, 0.0, device=device)
+
+    # ---- e2e: host buffers through the C ABI, copies inside the timed region
+    n = w.n
+    hp = torch.empty((n, 3), dtype=torch.float32).pin_memory()
+    hv = torch.empty((n, 3), dtype=torch.float32).pin_memory()
+    ht = torch.empty((n,), dtype=torch.int32).pin_memory()
+    R, st = sim.get_state_ptrs(hp.data_ptr(), hv.data_ptr(), ht.data_ptr(), 0)
+    ke = args.e2e_steps if args.e2e_steps > 0 else args.steps
+
+    def e2e_loop(k, st):
+        for _ in range(k):
+            sim.set_state_ptrs(hp.data_ptr(), hv.data_ptr(), ht.data_ptr(), st, 0)
+            sim.step(1)
+            _, st = sim.get_state_ptrs(hp.data_ptr(), hv.data_ptr(), ht.data_ptr(), 0)
+        return st
+
+    st = e2e_loop(3, st)
+    replicas.barrier()
+    torch.cuda.synchronize()
+    e0.record(sim.stream)
+    t0 = time.perf_counter()
+    st = e2e_loop(ke, st)
+    e1.record(sim.stream)
+    e1.synchronize()
+    e2e_wall_ms = (time.perf_counter() - t0) * 1e3
+    e2e_ms = max(e0.elapsed_time(e1), e2e_wall_ms)
+    replicas.barrier()
+    e2e_max, e2e_units = replicas.reduce_timing(e2e_ms, float(n) * ke, device=device)
+
+    # ---- roofline of the dominant kernel (pair force) ----------------------
+    force_ms = stages["pair_force"] / args.steps
+    pairs = 0.5 * (pairs0 + pairs1)
+    flops = FLOP_PER_PAIR * pairs
+    peak_tflops = n_sms * FP32_LANES_PER_SM * 2 * pk["sm_max_mhz"] * 1e6 * 1e-12
+    achieved = flops / (force_ms * 1e-3) * 1e-12
+    roofline = {
+        "kernel": "k_pair_force", "bound": "alu",
+        "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s",
+        "frac": achieved / peak_tflops,
+        "traffic": args.force_traffic_bytes,
+        "peak_source": f"{n_sms} SMs x 128 FP32 lanes x 2 x {pk['sm_max_mhz']:.0f} MHz "
+                       f"(DESIGN.md); measured FMA microkernel {fma_tflops:.1f} TFLOP/s",
+        "algorithmic_flops_per_launch": flops,
+        "in_range_ordered_pairs": pairs, "flop_per_pair": FLOP_PER_PAIR,
+        "kernel_ms": force_ms,
+        "share_of_step": stages["pair_force"] / tot_ms,
+        "hbm_algorithmic_gbs": 32.0 * n / (force_ms * 1e-3) * 1e-9,
+        "hbm_peak_gbs": pk["hbm_gbs"],
+    }
+
+    out = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms_max / args.steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": f"{w.name} (BASELINE.json configs[{int(w.name[1]) - 1}]): N={n}, "
+                               f"{w.n_types} types, steps {args.start_step + 0}.. of the schedule",
+                   "n_particles": n, "start_step": args.start_step,
+                   "replicas": world, "parallelism": "independent replicas, no collective",
+                   "l2": "flushed between timed steps (256 MiB memset on the same stream)",
+                   "timing": "CUDA events on the library's stream around every step; sum over K"},
+        "clocks": clocks,
+        "gpu_launches": launches_per_step * args.steps,
+        "launches_per_step": launches_per_step,
+        "stage_ms_per_step": {k: v / args.steps for k, v in stages.items()},
+        "wall_s_timed_region": wall_s,
+        "roofline": roofline,
+        "resident": {"value": float(n) * args.steps * world / (res_max * 1e-3), "unit": UNIT,
+                     "ms_per_step": res_max / args.steps,
+                     "how": "lv_step(K) as CUDA-graph replay, no L2 flush, events around the K steps"},
+        "e2e": {"value": e2e_units / (e2e_max * 1e-3), "unit": UNIT, "steps": ke,
+                "h2d_bytes_per_step": 28 * n, "d2h_bytes_per_step": 28 * n + 16,
+                "ms_per_step": e2e_max / ke,
+                "how": "lv_set_state(host pinned) + lv_step(1) + lv_get_state(host pinned) per step"},
+    }
+
+    # ---- further points of the schedule (not the headline) -----------------
+    if rank == 0 and world == 1 and args.snapshots:
+        snaps = []
+        for target in args.snapshots:
+            _, _, _, _, cur = sim.get_state()
+            if target < cur:
+                continue
+            sim.step(target - cur)
+            _, _, _, Rn, cur = sim.get_state()
+            sg, tt, pp = measure_point(sim, torch, flush, w, args.snapshot_steps, 10)
+            fm = sg["pair_force"] / args.snapshot_steps
+            snaps.append({"step": cur, "R": Rn,
+                          "value": float(n) * args.snapshot_steps / (tt * 1e-3),
+                          "ms_per_step": tt / args.snapshot_steps,
+                          "pair_force_ms": fm, "in_range_ordered_pairs": pp,
+                          "roofline_frac": FLOP_PER_PAIR * pp / (fm * 1e-3) * 1e-12 / peak_tflops})
+        out["snapshots"] = snaps
+
+    # ---- oracle beside it (rank 0, N = 1 only) -----------------------------
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        out["cpu_baseline"] = cpu_baseline(args.workload, args.cpu_seconds)
+    sim.close()
+    if rank == 0:
+        print(json.dumps(out))
+
+
+# ------------------------------------------------------------ oracle timing
+def cpu_baseline(name, budget_s):
+    """The oracle as it stands on the host cores: full-size steps of the same
+    workload from its initial state until ~budget_s of work is done."""
+    import oracle
+    w = workloads.make_workload(name)
+    p = oracle.params_from_workload(w)
+    x, v = w.pos.astype(np.float64), w.vel.astype(np.float64)
+    t0 = time.perf_counter()
+    x, v, bad = oracle.step(p, x, v, w.type, step0=0, nsteps=1)
+    t1 = time.perf_counter() - t0
+    m = int(max(1, min(50, budget_s / max(t1, 1e-3))))
+    t0 = time.perf_counter()
+    x, v, bad = oracle.step(p, x, v, w.type, step0=1, nsteps=m)
+    dt = time.perf_counter() - t0
+    return {"value": w.n * m / dt, "unit": UNIT, "cores": oracle.max_threads(), "kind": "oracle",
+            "sample": f"{m} full-size steps (N={w.n}) of {w.name} from its initial state, "
+                      f"fp64, OpenMP over particles, {dt:.1f} s",
+            "ms_per_step": dt / m * 1e3}
+
+
+def run_reference(args):
+    rank, _, world = replicas.env_rank_world()
+    if rank != 0:
+        return
+    import oracle
+    w = workloads.make_workload(args.workload)
+    n = w.n
+    p = oracle.params_from_workload(w)
+    x, v = w.pos.astype(np.float64), w.vel.astype(np.float64)
+    t0 = time.perf_counter()
+    x, v, _ = oracle.step(p, x, v, w.type, step0=0, nsteps=1)
+    t1 = time.perf_counter() - t0
+    total = args.steps + args.warmup
+    sample = f"full-size steps (N={n})"
+    if t1 * total > args.reference_budget_s:
+        # bounded sample: a scaled-down copy of the workload at the same volume
+        # fractions (workloads.make_workload(name, n)), so a step costs the same per particle
+        n = max(2048, int(n * args.reference_budget_s / (t1 * total)))
+        w = workloads.make_workload(args.workload, n)
+        p = oracle.params_from_workload(w)
+        x, v = w.pos.astype(np.float64), w.vel.astype(np.float64)
+        sample = f"scaled-down copy with N={n} at the same volume fractions"
+        done = 0
+    else:
+        done = 1
+    step = done
+    for _ in range(max(args.warmup - done, 0)):
+        x, v, _ = oracle.step(p, x, v, w.type, step0=step, nsteps=1)
+        step += 1
+    t0 = time.perf_counter()
+    x, v, bad = oracle.step(p, x, v, w.type, step0=step, nsteps=args.steps)
+    dt = time.perf_counter() - t0
+    value = n * args.steps / dt
+    out = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic",
+        "config": {"workload": f"{w.name}: {sample}", "n_particles": n, "start_step": 0},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": oracle.max_threads(),
+                         "kind": "oracle", "sample": f"{args.steps} {sample} of {w.name}, fp64"},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(out))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=500)
+    ap.add_argument("--warmup", type=int, default=50)
+    ap.add_argument("--impl", default="lv", choices=["lv", "reference"])
+    ap.add_argument("--workload", default="C3")
+    ap.add_argument("--start-step", type=int, default=0)
+    ap.add_argument("--cells-per-cut", type=int, nargs="*", default=None)
+    ap.add_argument("--e2e-steps", type=int, default=0)
+    ap.add_argument("--snapshots", type=int, nargs="*", default=[10000, 17000])
+    ap.add_argument("--snapshot-steps", type=int, default=100)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-seconds", type=float, default=15.0)
+    ap.add_argument("--reference-budget-s", type=float, default=150.0)
+    ap.add_argument("--force-traffic-bytes", type=float, default=None,
+                    help="dram bytes per launch of the force kernel from the committed ncu capture")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_lv(args)
+
+
+if __name__ == "__main__":
+    main()
