@@ -23,7 +23,7 @@
  *     in sm_100a kernels of this library.  There is no CPU fallback.
  *   - State is fp32; tables are derived on the host in fp64 and rounded once.
  *   - Call order: lv_create -> lv_set_types [-> lv_set_forces]
- *     [-> lv_set_droplet_schedule] [-> lv_set_grid] -> lv_workspace_bytes ->
+ *     [-> lv_set_droplet_schedule] [-> lv_set_grid] [-> lv_set_option] -> lv_workspace_bytes ->
  *     lv_bind -> lv_set_state -> lv_step / lv_compute_forces / lv_get_* ...
  *     -> lv_destroy.  A setter called after lv_bind returns LV_E_ORDER.
  */
@@ -99,7 +99,7 @@ typedef struct {
  * a, b: host, written. */
 int lv_langevin_coeffs(double gamma, double kT, double mass, double dt, double *a, double *b);
 
-/* Allocate a handle (host) for n NPs of n_types types (1..LV_MAX_TYPES).
+/* Allocate a handle (host) for n NPs (0 <= n < 2^28) of n_types types (1..LV_MAX_TYPES).
  * seed keys the Philox4x32-10 noise (R15); dt is the time step. */
 int lv_create(lv_sim **out, int n, int n_types, uint64_t seed, double dt);
 
@@ -131,6 +131,24 @@ int lv_set_droplet_schedule(lv_sim *s, int mode, double R0, double R1, int64_t n
 /* Optional: cells per cut-off k_b >= 1 for the grid of each type (host
  * [n_types]); cell edge h_b = r_c,bb (1 + 2^-9) / k_b.  Default 1. */
 int lv_set_grid(lv_sim *s, const int32_t *cells_per_cut);
+
+/* Implementation choices that do not change any result (tests check that):
+ *   LV_OPT_SORT          LV_SORT_COUNTING (default): the cell sort as a radix sort
+ *                        whose single digit is the whole key -- histogram, scan,
+ *                        stable scatter (4 kernels); LV_SORT_RADIX: the on-board
+ *                        multi-pass LSD radix sort (CUB) + offsets/scatter kernel.
+ *   LV_OPT_FORCE_KERNEL  LV_FORCE_QUEUED (default): test phase / force phase with
+ *                        per-thread in-range queues; LV_FORCE_SIMPLE: the first
+ *                        kernel (inline force), kept as the measured baseline.
+ * Both settings of either option give bit-identical permutations, offsets and
+ * neighbour counts; forces agree to rounding (identical summation order). */
+#define LV_OPT_SORT          1
+#define LV_OPT_FORCE_KERNEL  2
+#define LV_SORT_COUNTING     0
+#define LV_SORT_RADIX        1
+#define LV_FORCE_SIMPLE      0
+#define LV_FORCE_QUEUED      1
+int lv_set_option(lv_sim *s, int option, int value);
 
 /* Bytes of device workspace lv_bind needs (0 if types are not set). */
 size_t lv_workspace_bytes(const lv_sim *s);
@@ -183,7 +201,8 @@ int lv_launches_per_step(const lv_sim *s);
 /* Measurement aid: take ONE step exactly like lv_step(1) (same kernels, direct
  * launches instead of the graph) with CUDA events between the stages on the
  * stream, synchronise, and write the device time of each stage in
- * milliseconds to ms_out (host[LV_N_STAGES]): hash, sort, offsets+scatter,
+ * milliseconds to ms_out (host[LV_N_STAGES]): hash (+ histogram), sort (radix
+ * passes, or the histogram scan), offsets+scatter (or place + rank/gather),
  * pair force, update. */
 #define LV_N_STAGES 5
 int lv_step_profiled(lv_sim *s, float *ms_out);

@@ -22,10 +22,13 @@ WALL_ONESIDED, WALL_WINDOW = 0, 1
 ST_NONFINITE, ST_OUTSIDE_GRID = 1, 2
 DBG_KEYS, DBG_KEYS_SORTED, DBG_PERM, DBG_CELL_OFFSETS, DBG_IDS_SORTED, DBG_GRID = 1, 2, 3, 4, 5, 6
 E_NONFINITE = -5
+OPT_SORT, OPT_FORCE_KERNEL = 1, 2
+SORT_COUNTING, SORT_RADIX = 0, 1
+FORCE_SIMPLE, FORCE_QUEUED = 0, 1
 
 # every symbol include/lv.h declares (tests check the library exports them all)
 SYMBOLS = ["lv_langevin_coeffs", "lv_create", "lv_set_types", "lv_set_forces",
-           "lv_set_droplet_schedule", "lv_set_grid", "lv_workspace_bytes", "lv_bind",
+           "lv_set_droplet_schedule", "lv_set_grid", "lv_set_option", "lv_workspace_bytes", "lv_bind",
            "lv_set_state", "lv_step", "lv_compute_forces", "lv_get_state", "lv_get_forces",
            "lv_get_status", "lv_get_debug", "lv_launches_per_step", "lv_step_profiled",
            "lv_stage_timing", "lv_read_stage_timing",
@@ -69,6 +72,7 @@ def load():
     L.lv_set_forces.argtypes = [vp, C.c_double, dp, C.c_int]
     L.lv_set_droplet_schedule.argtypes = [vp, C.c_int, C.c_double, C.c_double, C.c_int64]
     L.lv_set_grid.argtypes = [vp, ip]
+    L.lv_set_option.argtypes = [vp, C.c_int, C.c_int]
     L.lv_workspace_bytes.argtypes = [vp]
     L.lv_workspace_bytes.restype = C.c_size_t
     L.lv_bind.argtypes = [vp, vp, C.c_size_t, vp]
@@ -153,6 +157,9 @@ class Simulation:
     def set_grid(self, cells_per_cut):
         k = np.ascontiguousarray(cells_per_cut, dtype=np.int32)
         self._check(self.L.lv_set_grid(self.h, k.ctypes.data_as(C.POINTER(C.c_int32))), "lv_set_grid")
+
+    def set_option(self, option: int, value: int):
+        self._check(self.L.lv_set_option(self.h, int(option), int(value)), "lv_set_option")
 
     def workspace_bytes(self) -> int:
         return int(self.L.lv_workspace_bytes(self.h))
@@ -301,7 +308,8 @@ class Simulation:
 
     # -- convenience -----------------------------------------------------------
     @classmethod
-    def from_workload(cls, w, cells_per_cut=None, device="cuda:0", load_state=True) -> "Simulation":
+    def from_workload(cls, w, cells_per_cut=None, device="cuda:0", load_state=True,
+                      options=None) -> "Simulation":
         """Configure from a workloads.Workload: per-type (a, b) through
         lv_langevin_coeffs, Lorentz-Berthelot tables inside lv_set_types."""
         sim = cls(w.n, w.n_types, w.seed, w.dt, device=device)
@@ -315,6 +323,8 @@ class Simulation:
         sim.set_droplet_schedule(w.sched_mode, w.R0, w.R1, w.sched_steps)
         if cells_per_cut is not None:
             sim.set_grid(cells_per_cut)
+        for opt, val in (options or {}).items():
+            sim.set_option(opt, val)
         sim.bind()
         if load_state:
             sim.set_state(w.pos, w.vel, w.type, 0)

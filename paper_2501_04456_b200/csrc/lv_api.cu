@@ -27,6 +27,8 @@ struct lv_sim {
     double R0 = 0.0, R1 = 0.0;
     int64_t sched_steps = 0;
     int32_t cells_per_cut[LV_MAX_TYPES];
+    int sort_mode = LV_SORT_COUNTING;
+    int force_kernel = LV_FORCE_QUEUED;
     lv_grid_info grid;
     int sort_end_bit = 1;
     size_t ws_bytes = 0;
@@ -99,7 +101,7 @@ int derive_grid(lv_sim *s)
 
 struct Layout {
     size_t posA, velA, posB, velB, force, key_in, key_out, val_in, val_out, cell_off, sort_temp,
-        sort_temp_bytes, st, staging, total;
+        sort_temp_bytes, st, staging, cell_cnt, scan_tile, scan_ticket, total;
 };
 
 Layout layout_of(const lv_sim *s)
@@ -113,7 +115,11 @@ Layout layout_of(const lv_sim *s)
     L.force = take(16 * n);
     L.key_in = take(4 * n); L.key_out = take(4 * n);
     L.val_in = take(4 * n); L.val_out = take(4 * n);
-    L.cell_off = take(4 * ((size_t)s->grid.base[s->n_types] + 1));
+    const size_t n_cells1 = (size_t)s->grid.base[s->n_types] + 1;
+    L.cell_off = take(4 * n_cells1);
+    L.cell_cnt = take(4 * n_cells1);
+    L.scan_tile = take(8 * ((n_cells1 + kScanTile - 1) / kScanTile));
+    L.scan_ticket = take(4);
     L.sort_temp_bytes = lvs_temp_bytes(s->n, s->sort_end_bit);
     L.sort_temp = take(L.sort_temp_bytes);
     L.st = take(sizeof(LvDevState));
@@ -130,6 +136,7 @@ void derive_tables(lv_sim *s)
     d.n = s->n;
     d.n_types = T;
     d.n_cells = s->grid.base[T];
+    d.n_scan_tiles = (uint32_t)(((size_t)d.n_cells + 1 + kScanTile - 1) / kScanTile);
     d.wall_mode = s->wall_mode;
     for (int a = 0; a < T; ++a)
         for (int b = 0; b < T; ++b) {
@@ -166,15 +173,48 @@ void derive_tables(lv_sim *s)
     d.seed_hi = (uint32_t)(s->seed >> 32);
 }
 
-// steps (i)-(ii): hash -> sort -> offsets + scatter -> pair force
+// The stages of one step, in order (LV_N_STAGES = 5).  Radix mode: hash | CUB radix
+// sort | offsets + scatter | pair force | update.  Counting mode (default): hash +
+// histogram | scan (= cell offsets) | place + rank/gather | pair force | update.
+int enqueue_stage(lv_sim *s, int stage)
+{
+    const bool counting = s->sort_mode == LV_SORT_COUNTING;
+    switch (stage) {
+    case 0:
+        if (counting) LV_CUDA(s, lvk_hash_count(s->dev, s->bufs, s->stream));
+        else LV_CUDA(s, lvk_hash(s->dev, s->bufs, s->stream));
+        break;
+    case 1:
+        if (counting) LV_CUDA(s, lvk_scan_cells(s->dev, s->bufs, s->stream));
+        else LV_CUDA(s, lvs_sort_pairs(s->bufs.sort_temp, s->bufs.sort_temp_bytes, s->bufs.key_in,
+                                       s->bufs.key_out, s->bufs.val_in, s->bufs.val_out, s->n,
+                                       s->sort_end_bit, s->stream));
+        break;
+    case 2:
+        if (counting) {
+            LV_CUDA(s, lvk_place(s->dev, s->bufs, s->stream));
+            LV_CUDA(s, lvk_rank_gather(s->dev, s->bufs, s->stream));
+        } else {
+            LV_CUDA(s, lvk_bounds_scatter(s->dev, s->bufs, s->stream));
+        }
+        break;
+    case 3:
+        LV_CUDA(s, lvk_pair_force(s->dev, s->bufs, s->force_kernel, s->stream));
+        break;
+    default:
+        LV_CUDA(s, lvk_update(s->dev, s->bufs, s->stream));
+        break;
+    }
+    return LV_OK;
+}
+
+// steps (i)-(ii): cell rebuild -> pair force
 int enqueue_rebuild_and_forces(lv_sim *s)
 {
-    LV_CUDA(s, lvk_hash(s->dev, s->bufs, s->stream));
-    LV_CUDA(s, lvs_sort_pairs(s->bufs.sort_temp, s->bufs.sort_temp_bytes, s->bufs.key_in,
-                              s->bufs.key_out, s->bufs.val_in, s->bufs.val_out, s->n,
-                              s->sort_end_bit, s->stream));
-    LV_CUDA(s, lvk_bounds_scatter(s->dev, s->bufs, s->stream));
-    LV_CUDA(s, lvk_pair_force(s->dev, s->bufs, s->stream));
+    for (int k = 0; k < 4; ++k) {
+        int rc = enqueue_stage(s, k);
+        if (rc != LV_OK) return rc;
+    }
     return LV_OK;
 }
 
@@ -182,26 +222,18 @@ int enqueue_step(lv_sim *s)
 {
     int rc = enqueue_rebuild_and_forces(s);
     if (rc != LV_OK) return rc;
-    LV_CUDA(s, lvk_update(s->dev, s->bufs, s->stream));
-    return LV_OK;
+    return enqueue_stage(s, 4);
 }
 
 // One step as direct launches with an event before the first and after each stage.
 int enqueue_step_timed(lv_sim *s, cudaEvent_t *ev)
 {
     LV_CUDA(s, cudaEventRecord(ev[0], s->stream));
-    LV_CUDA(s, lvk_hash(s->dev, s->bufs, s->stream));
-    LV_CUDA(s, cudaEventRecord(ev[1], s->stream));
-    LV_CUDA(s, lvs_sort_pairs(s->bufs.sort_temp, s->bufs.sort_temp_bytes, s->bufs.key_in,
-                              s->bufs.key_out, s->bufs.val_in, s->bufs.val_out, s->n,
-                              s->sort_end_bit, s->stream));
-    LV_CUDA(s, cudaEventRecord(ev[2], s->stream));
-    LV_CUDA(s, lvk_bounds_scatter(s->dev, s->bufs, s->stream));
-    LV_CUDA(s, cudaEventRecord(ev[3], s->stream));
-    LV_CUDA(s, lvk_pair_force(s->dev, s->bufs, s->stream));
-    LV_CUDA(s, cudaEventRecord(ev[4], s->stream));
-    LV_CUDA(s, lvk_update(s->dev, s->bufs, s->stream));
-    LV_CUDA(s, cudaEventRecord(ev[5], s->stream));
+    for (int k = 0; k < LV_N_STAGES; ++k) {
+        int rc = enqueue_stage(s, k);
+        if (rc != LV_OK) return rc;
+        LV_CUDA(s, cudaEventRecord(ev[k + 1], s->stream));
+    }
     return LV_OK;
 }
 
@@ -266,7 +298,7 @@ int lv_langevin_coeffs(double gamma, double kT, double mass, double dt, double *
 
 int lv_create(lv_sim **out, int n, int n_types, uint64_t seed, double dt)
 {
-    if (!out || n < 0 || n_types < 1 || n_types > LV_MAX_TYPES || !(dt > 0.0)) return LV_E_ARG;
+    if (!out || n < 0 || n >= (1 << 28) || n_types < 1 || n_types > LV_MAX_TYPES || !(dt > 0.0)) return LV_E_ARG;
     lv_sim *s = new (std::nothrow) lv_sim();
     if (!s) return LV_E_NOMEM;
     s->n = n;
@@ -347,6 +379,24 @@ int lv_set_grid(lv_sim *s, const int32_t *cells_per_cut)
     return LV_OK;
 }
 
+int lv_set_option(lv_sim *s, int option, int value)
+{
+    if (!s) return LV_E_ARG;
+    if (s->bound) return LV_E_ORDER;
+    switch (option) {
+    case LV_OPT_SORT:
+        if (value != LV_SORT_COUNTING && value != LV_SORT_RADIX) return LV_E_ARG;
+        s->sort_mode = value;
+        return LV_OK;
+    case LV_OPT_FORCE_KERNEL:
+        if (value != LV_FORCE_QUEUED && value != LV_FORCE_SIMPLE) return LV_E_ARG;
+        s->force_kernel = value;
+        return LV_OK;
+    default:
+        return LV_E_ARG;
+    }
+}
+
 size_t lv_workspace_bytes(const lv_sim *cs)
 {
     lv_sim *s = const_cast<lv_sim *>(cs);
@@ -377,10 +427,15 @@ int lv_bind(lv_sim *s, void *workspace_dev, size_t workspace_bytes, void *cuda_s
     B.sort_temp_bytes = L.sort_temp_bytes;
     B.st = (LvDevState *)(w + L.st);
     B.staging = w + L.staging;
+    B.cell_cnt = (uint32_t *)(w + L.cell_cnt);
+    B.scan_tile = (unsigned long long *)(w + L.scan_tile);
+    B.scan_ticket = (unsigned int *)(w + L.scan_ticket);
     s->ws_bytes = L.total;
     s->stream = (cudaStream_t)cuda_stream;
     derive_tables(s);
     LV_CUDA(s, cudaMemsetAsync(B.st, 0, sizeof(LvDevState), s->stream));
+    // the histogram is zero between steps: the scan clears what it has read
+    LV_CUDA(s, cudaMemsetAsync(B.cell_cnt, 0, 4 * ((size_t)s->grid.base[s->n_types] + 1), s->stream));
     rc = build_graph(s);
     if (rc != LV_OK) return rc;
     s->bound = true;
@@ -522,7 +577,14 @@ int lv_get_debug(lv_sim *s, int what, void *dst, size_t bytes, int on_device)
     case LV_DBG_KEYS:
         rc = copy_out(s, dst, s->bufs.key_in, bytes < 4 * n ? bytes : 4 * n, on_device); break;
     case LV_DBG_KEYS_SORTED:
-        rc = copy_out(s, dst, s->bufs.key_out, bytes < 4 * n ? bytes : 4 * n, on_device); break;
+        if (s->sort_mode == LV_SORT_COUNTING) {
+            if (n == 0) break;
+            LV_CUDA(s, lvk_keys_sorted(s->dev, s->bufs, (uint32_t *)s->bufs.staging, s->stream));
+            rc = copy_out(s, dst, s->bufs.staging, bytes < 4 * n ? bytes : 4 * n, on_device);
+        } else {
+            rc = copy_out(s, dst, s->bufs.key_out, bytes < 4 * n ? bytes : 4 * n, on_device);
+        }
+        break;
     case LV_DBG_PERM:
         rc = copy_out(s, dst, s->bufs.val_out, bytes < 4 * n ? bytes : 4 * n, on_device); break;
     case LV_DBG_CELL_OFFSETS: {
@@ -553,23 +615,16 @@ int lv_step_profiled(lv_sim *s, float *ms_out)
     for (int k = 0; k <= LV_N_STAGES; ++k) LV_CUDA(s, cudaEventCreate(&ev[k]));
     int rc = LV_OK;
     cudaError_t e = cudaSuccess;
-#define LV_STAGE(k, call)                                         \
-    if (e == cudaSuccess) e = (call);                             \
-    if (e == cudaSuccess) e = cudaEventRecord(ev[(k) + 1], s->stream);
     e = cudaEventRecord(ev[0], s->stream);
-    LV_STAGE(0, lvk_hash(s->dev, s->bufs, s->stream));
-    LV_STAGE(1, lvs_sort_pairs(s->bufs.sort_temp, s->bufs.sort_temp_bytes, s->bufs.key_in,
-                               s->bufs.key_out, s->bufs.val_in, s->bufs.val_out, s->n,
-                               s->sort_end_bit, s->stream));
-    LV_STAGE(2, lvk_bounds_scatter(s->dev, s->bufs, s->stream));
-    LV_STAGE(3, lvk_pair_force(s->dev, s->bufs, s->stream));
-    LV_STAGE(4, lvk_update(s->dev, s->bufs, s->stream));
-#undef LV_STAGE
+    for (int k = 0; k < LV_N_STAGES && e == cudaSuccess && rc == LV_OK; ++k) {
+        rc = enqueue_stage(s, k);
+        if (rc == LV_OK) e = cudaEventRecord(ev[k + 1], s->stream);
+    }
     if (e == cudaSuccess) e = cudaStreamSynchronize(s->stream);
-    for (int k = 0; e == cudaSuccess && k < LV_N_STAGES; ++k)
+    for (int k = 0; rc == LV_OK && e == cudaSuccess && k < LV_N_STAGES; ++k)
         e = cudaEventElapsedTime(&ms_out[k], ev[k], ev[k + 1]);
     for (int k = 0; k <= LV_N_STAGES; ++k) cudaEventDestroy(ev[k]);
-    if (e != cudaSuccess) rc = cuda_fail(s, e, "lv_step_profiled");
+    if (rc == LV_OK && e != cudaSuccess) rc = cuda_fail(s, e, "lv_step_profiled");
     return rc;
 }
 

@@ -46,6 +46,7 @@ struct LvDev {
     double wall_k_d[LV_MAX_TYPES];
     double radius_d[LV_MAX_TYPES];
     uint32_t seed_lo, seed_hi;
+    uint32_t n_scan_tiles;   // tiles of the cell-count scan (counting sort)
 };
 
 // Device-resident scalars.
@@ -59,8 +60,14 @@ struct LvBufs {
     float4 *posA, *velA;   // current state, slot order of the last rebuild (w: type / id bits)
     float4 *posB, *velB;   // cell-sorted copy of the current step
     float4 *force;         // pair force per sorted slot (w: in-range count bits)
+    // key_in: cell key per current slot.  Radix mode: val_in = slot, key_out / val_out =
+    // sorted keys / permutation.  Counting mode: val_in = arrival rank inside the cell,
+    // key_out = per-cell slot lists in arrival order, val_out = permutation.
     uint32_t *key_in, *key_out, *val_in, *val_out;
     uint32_t *cell_off;    // [n_cells + 1]
+    uint32_t *cell_cnt;    // [n_cells + 1] NPs per cell; zero between steps (counting mode)
+    unsigned long long *scan_tile;   // [n_scan_tiles] look-back words of the scan
+    unsigned int *scan_ticket;
     void *sort_temp;
     size_t sort_temp_bytes;
     LvDevState *st;
@@ -78,10 +85,18 @@ __host__ __device__ inline double lv_radius_of(int mode, double R0, double R1, l
     return sqrt(R0 * R0 + (R1 * R1 - R0 * R0) * f);
 }
 
+constexpr int kScanTile = 4096;   // cells per tile of the cell-count scan
+
 // ---- launch wrappers (lv_kernels.cu) -- all asynchronous on `st` ----------
 cudaError_t lvk_hash(const LvDev &P, const LvBufs &B, cudaStream_t st);
 cudaError_t lvk_bounds_scatter(const LvDev &P, const LvBufs &B, cudaStream_t st);
-cudaError_t lvk_pair_force(const LvDev &P, const LvBufs &B, cudaStream_t st);
+// counting sort (one radix digit = the whole key): hash + count, scan, place, rank + gather
+cudaError_t lvk_hash_count(const LvDev &P, const LvBufs &B, cudaStream_t st);
+cudaError_t lvk_scan_cells(const LvDev &P, const LvBufs &B, cudaStream_t st);
+cudaError_t lvk_place(const LvDev &P, const LvBufs &B, cudaStream_t st);
+cudaError_t lvk_rank_gather(const LvDev &P, const LvBufs &B, cudaStream_t st);
+cudaError_t lvk_keys_sorted(const LvDev &P, const LvBufs &B, uint32_t *out, cudaStream_t st);
+cudaError_t lvk_pair_force(const LvDev &P, const LvBufs &B, int variant, cudaStream_t st);
 cudaError_t lvk_update(const LvDev &P, const LvBufs &B, cudaStream_t st);
 cudaError_t lvk_pack_state(const LvDev &P, const LvBufs &B, const float *pos, const float *vel,
                            const int32_t *type, long long step, cudaStream_t st);

@@ -89,6 +89,156 @@ k_bounds_scatter(const __grid_constant__ LvDev P, const uint32_t *__restrict__ k
     warp_fill(off, tail_first, tail_count, (uint32_t)P.n, lane);
 }
 
+// ------------------------------------- A2-A5 as ONE-digit radix (counting) sort
+// The key has ceil(log2 n_cells) bits; a radix sort whose single digit spans the
+// whole key is a counting sort: histogram (k_hash_count), exclusive scan of the
+// histogram (k_scan_cells: this IS the cell-offset table of A4), scatter.  The
+// scatter is made stable -- ties keep slot order, fp32 contract #3 -- in two
+// steps: k_place drops every slot into its cell's segment in arrival order
+// (atomic rank, any order), k_rank_gather replaces arrival order by the rank of
+// the slot index inside the segment and moves the state (A5).
+__global__ void __launch_bounds__(kThreads)
+k_hash_count(const __grid_constant__ LvDev P, const float4 *__restrict__ pos,
+             uint32_t *__restrict__ key, uint32_t *__restrict__ rank, uint32_t *__restrict__ cnt,
+             unsigned long long *__restrict__ scan_tile, unsigned int *__restrict__ scan_ticket,
+             LvDevState *st)
+{
+    int i = blockIdx.x * kThreads + threadIdx.x;
+    if (i < (int)P.n_scan_tiles) scan_tile[i] = 0ull;   // re-arm the scan that follows
+    if (i == 0) *scan_ticket = 0u;
+    if (i >= P.n) return;
+    float4 p = pos[i];
+    int b = __float_as_int(p.w);
+    const LvGridDev g = P.grid[b];
+    int cx = cell_coord(p.x, g.lo, g.inv_h, g.G);
+    int cy = cell_coord(p.y, g.lo, g.inv_h, g.G);
+    int cz = cell_coord(p.z, g.lo, g.inv_h, g.G);
+    const uint32_t k = g.base + (uint32_t)((cz * g.G + cy) * g.G + cx);
+    key[i] = k;
+    rank[i] = atomicAdd(cnt + k, 1u);
+    float hi = -g.lo;
+    bool outside = !(p.x >= g.lo && p.x < hi && p.y >= g.lo && p.y < hi && p.z >= g.lo && p.z < hi);
+    if (outside) atomicOr(&st->status, LV_ST_OUTSIDE_GRID);
+}
+
+// Exclusive scan of cnt[0 .. n_cells] into off[0 .. n_cells] (single pass, tiles
+// chained by decoupled look-back); cnt is zeroed behind the read so the next
+// step's histogram starts clean.  Look-back word = flag << 32 | value with
+// flag 1 = tile aggregate, 2 = inclusive prefix.
+constexpr int kScanThreads = 256;
+constexpr int kScanItems = kScanTile / kScanThreads;   // 16
+
+__global__ void __launch_bounds__(kScanThreads)
+k_scan_cells(uint32_t n_items, uint32_t *__restrict__ cnt, uint32_t *__restrict__ off,
+             volatile unsigned long long *scan_tile, unsigned int *scan_ticket)
+{
+    __shared__ uint32_t s_warp[kScanThreads / 32];
+    __shared__ uint32_t s_tile, s_excl;
+    if (threadIdx.x == 0) s_tile = atomicAdd(scan_ticket, 1u);   // tiles start in ticket order
+    __syncthreads();
+    const uint32_t tile = s_tile;
+    const uint32_t first = tile * kScanTile + threadIdx.x * kScanItems;
+    uint32_t v[kScanItems];
+    if (first + kScanItems <= n_items) {
+        uint4 *src = reinterpret_cast<uint4 *>(cnt + first);
+#pragma unroll
+        for (int q = 0; q < kScanItems / 4; ++q) {
+            uint4 t = src[q];
+            v[4 * q] = t.x; v[4 * q + 1] = t.y; v[4 * q + 2] = t.z; v[4 * q + 3] = t.w;
+            src[q] = make_uint4(0u, 0u, 0u, 0u);
+        }
+    } else {
+#pragma unroll
+        for (int q = 0; q < kScanItems; ++q) {
+            v[q] = 0u;
+            if (first + q < n_items) { v[q] = cnt[first + q]; cnt[first + q] = 0u; }
+        }
+    }
+    uint32_t sum = 0;
+#pragma unroll
+    for (int q = 0; q < kScanItems; ++q) { uint32_t t = v[q]; v[q] = sum; sum += t; }
+    // block-exclusive prefix of the thread sums
+    const unsigned lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    uint32_t inc = sum;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        uint32_t t = __shfl_up_sync(0xffffffffu, inc, d);
+        if (lane >= d) inc += t;
+    }
+    if (lane == 31) s_warp[wid] = inc;
+    __syncthreads();
+    uint32_t wbase = 0, total = 0;
+#pragma unroll
+    for (int k = 0; k < kScanThreads / 32; ++k) {
+        uint32_t t = s_warp[k];
+        if (k < (int)wid) wbase += t;
+        total += t;
+    }
+    if (threadIdx.x == 0) {
+        uint32_t excl = 0;
+        if (tile > 0) {
+            scan_tile[tile] = (1ull << 32) | total;
+            for (int p = (int)tile - 1; p >= 0; --p) {
+                unsigned long long w;
+                do { w = scan_tile[p]; } while ((w >> 32) == 0ull);
+                excl += (uint32_t)w;
+                if ((w >> 32) == 2ull) break;
+            }
+        }
+        scan_tile[tile] = (2ull << 32) | (unsigned long long)(excl + total);
+        s_excl = excl;
+    }
+    __syncthreads();
+    const uint32_t tbase = s_excl + wbase + (inc - sum);
+    if (first + kScanItems <= n_items) {
+        uint4 *dst = reinterpret_cast<uint4 *>(off + first);
+#pragma unroll
+        for (int q = 0; q < kScanItems / 4; ++q)
+            dst[q] = make_uint4(tbase + v[4 * q], tbase + v[4 * q + 1], tbase + v[4 * q + 2],
+                                tbase + v[4 * q + 3]);
+    } else {
+#pragma unroll
+        for (int q = 0; q < kScanItems; ++q)
+            if (first + q < n_items) off[first + q] = tbase + v[q];
+    }
+}
+
+__global__ void __launch_bounds__(kThreads)
+k_place(int n, const uint32_t *__restrict__ key, const uint32_t *__restrict__ rank,
+        const uint32_t *__restrict__ off, uint32_t *__restrict__ arrival)
+{
+    int i = blockIdx.x * kThreads + threadIdx.x;
+    if (i < n) arrival[off[key[i]] + rank[i]] = (uint32_t)i;
+}
+
+__global__ void __launch_bounds__(kThreads)
+k_rank_gather(int n, const uint32_t *__restrict__ key, const uint32_t *__restrict__ off,
+              const uint32_t *__restrict__ arrival, uint32_t *__restrict__ perm,
+              const float4 *__restrict__ posA, const float4 *__restrict__ velA,
+              float4 *__restrict__ posB, float4 *__restrict__ velB)
+{
+    int k = blockIdx.x * kThreads + threadIdx.x;
+    if (k >= n) return;
+    const uint32_t v = arrival[k];
+    const float4 p = posA[v], u = velA[v];
+    const uint32_t c = key[v];
+    const uint32_t s = off[c], e = off[c + 1];
+    uint32_t r = 0;
+    for (uint32_t t = s; t < e; ++t) r += (arrival[t] < v) ? 1u : 0u;
+    const uint32_t dst = s + r;      // stable: rank of the slot index inside the cell
+    perm[dst] = v;
+    posB[dst] = p;
+    velB[dst] = u;
+}
+
+__global__ void __launch_bounds__(kThreads)
+k_keys_sorted(int n, const uint32_t *__restrict__ key, const uint32_t *__restrict__ perm,
+              uint32_t *__restrict__ out)
+{
+    int k = blockIdx.x * kThreads + threadIdx.x;
+    if (k < n) out[k] = key[perm[k]];
+}
+
 // ------------------------------------------------------------ A6 pair force
 __device__ __forceinline__ float rcp_approx(float x)
 {
@@ -155,6 +305,148 @@ k_pair_force(const __grid_constant__ LvDev P, const float4 *__restrict__ pos,
             }
     }
     force[i] = make_float4(fx, fy, fz, __int_as_float(cnt));
+}
+
+// Variant 1 (default).  Still one thread per cell-sorted NP, but the warp walks
+// the rows of the stencil in lock-step and the work is split in two phases:
+//   test phase  -- branch-free: every lane tests kChunk candidates of its own row
+//                  per iteration (rows are padded to the longest row of the warp
+//                  by predication) and pushes the slots that pass contract #2
+//                  into a private queue in shared memory;
+//   force phase -- when some lane's queue is nearly full (or at the end) every
+//                  lane drains its queue: only in-range pairs reach the
+//                  rcp / rsqrt / LJ arithmetic, so that block no longer runs at
+//                  the ~10 % lane occupancy of an inline `if (r2 < rc2)`.
+// Neighbouring lanes are neighbouring NPs, so in lock-step their loads fall in
+// the same or adjacent 128-byte lines.  NPs are taken from the END of the sorted
+// order first: the types with the longest ranges (most candidates) sit there.
+constexpr int kFThreads = 128;
+constexpr int kQCap = 16;       // queue slots per thread (8 KB per block: leaves the L1 its room)
+constexpr int kChunk = 4;       // candidates per lane and iteration
+constexpr unsigned kFull = 0xffffffffu;
+
+// pos[.] if `take`, else (+inf, ?, ?, ?); one predicated LDG, no branch
+__device__ __forceinline__ float4 ld_pos_if(const float4 *p, bool take)
+{
+    // y, z, w stay unwritten when the load is skipped: with x = +inf the distance is
+    // +inf or NaN whatever they hold, and both fail `r2 < rc2`
+    float4 r;
+    r.x = __int_as_float(0x7f800000);
+    asm("{\n\t.reg .pred p;\n\tsetp.ne.s32 p, %5, 0;\n\t"
+        "@p ld.global.nc.v4.f32 {%0, %1, %2, %3}, [%4];\n\t}"
+        : "+f"(r.x), "=f"(r.y), "=f"(r.z), "=f"(r.w)
+        : "l"(p), "r"((int)take));
+    return r;
+}
+
+__global__ void __launch_bounds__(kFThreads)
+k_pair_force_q(const __grid_constant__ LvDev P, const float4 *__restrict__ pos,
+               const uint32_t *__restrict__ off, float4 *__restrict__ force)
+{
+    __shared__ LvPair s_pair[LV_MAX_TYPES * LV_MAX_TYPES];
+    __shared__ int8_t s_w[LV_MAX_TYPES * LV_MAX_TYPES];
+    __shared__ uint32_t s_q[kQCap * kFThreads];
+    if (threadIdx.x < LV_MAX_TYPES * LV_MAX_TYPES) {
+        s_pair[threadIdx.x] = P.pair[threadIdx.x];
+        s_w[threadIdx.x] = P.w[threadIdx.x];
+    }
+    __syncthreads();
+    const int i = P.n - 1 - (int)(blockIdx.x * kFThreads + threadIdx.x);
+    const bool live = i >= 0;
+    const float4 pi = live ? pos[i] : make_float4(0.f, 0.f, 0.f, 0.f);
+    const int a = live ? __float_as_int(pi.w) : 0;
+    uint32_t *q = s_q + threadIdx.x;
+    float fx = 0.f, fy = 0.f, fz = 0.f;
+    int cnt = 0;
+    // next free queue slot of this thread, as a 32-bit shared-memory address
+    const uint32_t q0 = (uint32_t)__cvta_generic_to_shared(q);
+    uint32_t qp = q0;
+
+    auto drain = [&]() {
+        const int qn = (int)((qp - q0) / (4u * kFThreads));
+        const int m = __reduce_max_sync(kFull, qn);
+        for (int t = 0; t < m; ++t) {
+            if (t < qn) {
+                const uint32_t e = q[t * kFThreads];
+                const uint32_t j = e & 0x0fffffffu;
+                if (j != (uint32_t)i) {
+                    const LvPair pr = s_pair[a * LV_MAX_TYPES + (int)(e >> 28)];
+                    const float4 pj = __ldg(pos + j);
+                    const float dx = __fsub_rn(pi.x, pj.x);
+                    const float dy = __fsub_rn(pi.y, pj.y);
+                    const float dz = __fsub_rn(pi.z, pj.z);
+                    const float r2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
+                    const float ir2 = rcp_approx(r2);
+                    const float ir6 = ir2 * ir2 * ir2;
+                    float f = (pr.c12 * ir6 - pr.c6) * ir6 * ir2;
+                    if (pr.qq != 0.0f) f = fmaf(pr.qq * ir2, rsqrt_approx(r2), f);
+                    fx = fmaf(f, dx, fx);
+                    fy = fmaf(f, dy, fy);
+                    fz = fmaf(f, dz, fz);
+                    ++cnt;
+                }
+            }
+        }
+        qp = q0;
+    };
+
+    for (int b = 0; b < P.n_types; ++b) {
+        const LvGridDev g = P.grid[b];
+        const int w = live ? (int)s_w[a * LV_MAX_TYPES + b] : -1;
+        const int W = __reduce_max_sync(kFull, w);
+        if (W < 0) continue;
+        const float rc2 = s_pair[a * LV_MAX_TYPES + b].rc2;
+        const int cx = cell_coord(pi.x, g.lo, g.inv_h, g.G);
+        const int cy = cell_coord(pi.y, g.lo, g.inv_h, g.G);
+        const int cz = cell_coord(pi.z, g.lo, g.inv_h, g.G);
+        const int x0 = max(cx - w, 0), x1 = min(cx + w, g.G - 1);
+        const uint32_t btag = (uint32_t)b << 28;
+        // bounds of row (dy, dz): [js, je) in sorted slots, empty if the lane has no such row
+        auto bounds = [&](int dy, int dz, uint32_t &js, uint32_t &je) {
+            const int y = cy + dy, z = cz + dz;
+            js = 0u; je = 0u;
+            if (abs(dy) <= w && abs(dz) <= w && (unsigned)y < (unsigned)g.G && (unsigned)z < (unsigned)g.G) {
+                const uint32_t row = g.base + (uint32_t)((z * g.G + y) * g.G);
+                js = __ldg(off + row + x0);
+                je = __ldg(off + row + x1 + 1);
+            }
+        };
+        int dy = -W, dz = -W;
+        uint32_t njs, nje;
+        bounds(dy, dz, njs, nje);
+        const int nrows = (2 * W + 1) * (2 * W + 1);
+        for (int r = 0; r < nrows; ++r) {
+            const uint32_t js = njs, je = nje;
+            if (++dy > W) { dy = -W; ++dz; }
+            if (r + 1 < nrows) bounds(dy, dz, njs, nje);      // prefetch the next row
+            const int len = (int)(je - js);
+            const int maxlen = __reduce_max_sync(kFull, len);
+            for (int t = 0; t < maxlen; t += kChunk) {
+                // all kChunk loads are issued before the first test (predicated, never
+                // branched): a lane without a candidate keeps x = +inf, so r2 = +inf
+                // fails the predicate on its own
+                const float4 *pp = pos + js + (uint32_t)t;
+                const uint32_t e0 = (js + (uint32_t)t) | btag;   // slot < 2^28: adding u cannot carry into the tag
+                float4 pj[kChunk];
+#pragma unroll
+                for (int u = 0; u < kChunk; ++u) pj[u] = ld_pos_if(pp + u, t + u < len);
+#pragma unroll
+                for (int u = 0; u < kChunk; ++u) {
+                    const float dx = __fsub_rn(pi.x, pj[u].x);
+                    const float dy2 = __fsub_rn(pi.y, pj[u].y);
+                    const float dz2 = __fsub_rn(pi.z, pj[u].z);
+                    const float r2 = __fmaf_rn(dz2, dz2, __fmaf_rn(dy2, dy2, __fmul_rn(dx, dx)));
+                    if (r2 < rc2) {
+                        asm volatile("st.shared.u32 [%0], %1;" :: "r"(qp), "r"(e0 + (uint32_t)u) : "memory");
+                        qp += 4u * kFThreads;
+                    }
+                }
+                if (__any_sync(kFull, qp > q0 + 4u * (kQCap - kChunk) * kFThreads)) drain();
+            }
+        }
+    }
+    drain();
+    if (live) force[i] = make_float4(fx, fy, fz, __int_as_float(cnt));
 }
 
 // ------------------------------------------------- A1 + A7 fused update
@@ -310,9 +602,47 @@ cudaError_t lvk_bounds_scatter(const LvDev &P, const LvBufs &B, cudaStream_t st)
     return cudaGetLastError();
 }
 
-cudaError_t lvk_pair_force(const LvDev &P, const LvBufs &B, cudaStream_t st)
+cudaError_t lvk_pair_force(const LvDev &P, const LvBufs &B, int variant, cudaStream_t st)
 {
-    k_pair_force<<<blocks_for(P.n), kThreads, 0, st>>>(P, B.posB, B.cell_off, B.force);
+    if (variant == 0)
+        k_pair_force<<<blocks_for(P.n), kThreads, 0, st>>>(P, B.posB, B.cell_off, B.force);
+    else
+        k_pair_force_q<<<(P.n + kFThreads - 1) / kFThreads, kFThreads, 0, st>>>(P, B.posB, B.cell_off,
+                                                                             B.force);
+    return cudaGetLastError();
+}
+
+cudaError_t lvk_hash_count(const LvDev &P, const LvBufs &B, cudaStream_t st)
+{
+    const int m = P.n > (int)P.n_scan_tiles ? P.n : (int)P.n_scan_tiles;
+    k_hash_count<<<blocks_for(m), kThreads, 0, st>>>(P, B.posA, B.key_in, B.val_in, B.cell_cnt,
+                                                     B.scan_tile, B.scan_ticket, B.st);
+    return cudaGetLastError();
+}
+
+cudaError_t lvk_scan_cells(const LvDev &P, const LvBufs &B, cudaStream_t st)
+{
+    k_scan_cells<<<P.n_scan_tiles, kScanThreads, 0, st>>>(P.n_cells + 1u, B.cell_cnt, B.cell_off,
+                                                          B.scan_tile, B.scan_ticket);
+    return cudaGetLastError();
+}
+
+cudaError_t lvk_place(const LvDev &P, const LvBufs &B, cudaStream_t st)
+{
+    k_place<<<blocks_for(P.n), kThreads, 0, st>>>(P.n, B.key_in, B.val_in, B.cell_off, B.key_out);
+    return cudaGetLastError();
+}
+
+cudaError_t lvk_rank_gather(const LvDev &P, const LvBufs &B, cudaStream_t st)
+{
+    k_rank_gather<<<blocks_for(P.n), kThreads, 0, st>>>(P.n, B.key_in, B.cell_off, B.key_out, B.val_out,
+                                                        B.posA, B.velA, B.posB, B.velB);
+    return cudaGetLastError();
+}
+
+cudaError_t lvk_keys_sorted(const LvDev &P, const LvBufs &B, uint32_t *out, cudaStream_t st)
+{
+    k_keys_sorted<<<blocks_for(P.n), kThreads, 0, st>>>(P.n, B.key_in, B.val_out, out);
     return cudaGetLastError();
 }
 

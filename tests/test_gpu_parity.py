@@ -356,3 +356,51 @@ def test_explicit_interaction_matrix(B, orc):
     assert np.array_equal(cg, co)
     assert force_error(Fg, Fo, So) <= FORCE_TOL
     sim.close()
+
+
+VARIANTS = [  # (sort, force kernel): lv_set_option; (0, 1) is the default path
+    (1, 0), (1, 1), (0, 0),
+]
+
+
+@pytest.mark.parametrize("name,n,cpc", [("C1", None, None), ("C3", 20000, [1, 2, 2]),
+                                         ("C4", 19999, [2]), ("C2", 8191, None)])
+def test_implementation_options_do_not_change_results(B, orc, name, n, cpc):
+    """lv_set_option: the multi-pass radix sort vs the one-digit (counting) sort
+    and the two force kernels give bit-identical cell structures and neighbour
+    counts, forces equal to rounding, and -- for the two sorts -- bit-identical
+    trajectories."""
+    w = workload(name, n)
+    p = orc.params_from_workload(w)
+    g = orc.grid_spec(p, cpc)
+    key, ks, perm, off = orc.cell_structures(g, w.pos, w.type)
+    Fo, So, co, _ = orc.pair_forces(p, w.pos, w.type, "cells")
+    ref = B.Simulation.from_workload(w, cells_per_cut=cpc)
+    ref.compute_forces()
+    F0, c0 = ref.get_forces()
+    ref.step(30)
+    x0, v0, _, _, _ = ref.get_state()
+    ids0 = ref.get_debug(B.DBG_IDS_SORTED)
+    ref.close()
+    for sort, fk in VARIANTS:
+        sim = B.Simulation.from_workload(w, cells_per_cut=cpc,
+                                         options={B.OPT_SORT: sort, B.OPT_FORCE_KERNEL: fk})
+        sim.compute_forces()
+        assert np.array_equal(sim.get_debug(B.DBG_KEYS), key)
+        assert np.array_equal(sim.get_debug(B.DBG_KEYS_SORTED), ks)
+        assert np.array_equal(sim.get_debug(B.DBG_PERM), perm)
+        assert np.array_equal(sim.get_debug(B.DBG_CELL_OFFSETS), off)
+        F, c = sim.get_forces()
+        assert np.array_equal(c, co)
+        assert force_error(F, Fo, So) <= FORCE_TOL
+        assert force_error(F, F0.astype(np.float64), So) <= 2e-6
+        sim.step(30)
+        x, v, _, _, st = sim.get_state()
+        assert st == 30
+        if fk == 1:          # same force kernel as the default: the sort must not matter at all
+            assert np.array_equal(x, x0) and np.array_equal(v, v0)
+            assert np.array_equal(sim.get_debug(B.DBG_IDS_SORTED), ids0)
+        else:
+            R = w.R0
+            assert np.abs(x.astype(np.float64) - x0).max() <= 1e-4 * R
+        sim.close()
