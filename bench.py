@@ -181,7 +181,9 @@ def run_lv(args):
 
     base = workloads.make_workload(args.workload, state=False)
     w = workloads.make_workload(args.workload, seed=replicas.replica_seed(base.seed, rank))
-    sim = binding.Simulation.from_workload(w, cells_per_cut=args.cells_per_cut, device=device)
+    options = None if args.force_kernel is None else {binding.OPT_FORCE_KERNEL: args.force_kernel}
+    sim = binding.Simulation.from_workload(w, cells_per_cut=args.cells_per_cut, device=device,
+                                           options=options)
     if args.start_step > 0:
         sim.step(args.start_step)
         sim.get_state()                      # synchronises; raises on a non-finite state
@@ -396,6 +398,8 @@ def main():
     ap.add_argument("--workload", default="C3")
     ap.add_argument("--start-step", type=int, default=0)
     ap.add_argument("--cells-per-cut", type=int, nargs="*", default=None)
+    ap.add_argument("--force-kernel", type=int, default=None,
+                    help="lv_set_option(LV_OPT_FORCE_KERNEL): 0 simple, 1 queued, 2 segments")
     ap.add_argument("--e2e-steps", type=int, default=0)
     ap.add_argument("--snapshots", type=int, nargs="*", default=[10000, 17000])
     ap.add_argument("--snapshot-steps", type=int, default=100)

@@ -148,6 +148,7 @@ int lv_set_grid(lv_sim *s, const int32_t *cells_per_cut);
 #define LV_SORT_RADIX        1
 #define LV_FORCE_SIMPLE      0
 #define LV_FORCE_QUEUED      1
+#define LV_FORCE_SEGMENTS    2
 int lv_set_option(lv_sim *s, int option, int value);
 
 /* Bytes of device workspace lv_bind needs (0 if types are not set). */

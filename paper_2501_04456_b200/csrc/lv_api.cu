@@ -389,7 +389,7 @@ int lv_set_option(lv_sim *s, int option, int value)
         s->sort_mode = value;
         return LV_OK;
     case LV_OPT_FORCE_KERNEL:
-        if (value != LV_FORCE_QUEUED && value != LV_FORCE_SIMPLE) return LV_E_ARG;
+        if (value < LV_FORCE_SIMPLE || value > LV_FORCE_SEGMENTS) return LV_E_ARG;
         s->force_kernel = value;
         return LV_OK;
     default:

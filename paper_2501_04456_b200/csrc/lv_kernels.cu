@@ -449,6 +449,187 @@ k_pair_force_q(const __grid_constant__ LvDev P, const float4 *__restrict__ pos,
     if (live) force[i] = make_float4(fx, fy, fz, __int_as_float(cnt));
 }
 
+// Variant 2 (LV_FORCE_SEGMENTS, default).  The ncu capture of variant 1
+// (profiles/r1b) shows the kernel bound by instruction issue: 14.6 warp
+// instructions per in-range pair, most of them row bookkeeping, padding of the
+// row-by-row lock step and candidates that fail the cut-off.  Two phases:
+//   row phase   -- for each row (dy, dz) of the stencil the lane lower-bounds its
+//                  distance to that row of cells from its own cell coordinates
+//                  (gap^2, in cell units); rows farther than r_c are skipped, the
+//                  others keep only the x-cells a sphere of radius r_c can reach,
+//                  [x - sqrt(r_c^2 - gap^2), x + ...].  The stencil becomes a
+//                  cell-resolution ball instead of a cube, which is what makes
+//                  cells_per_cut >= 2 pay.  Non-empty runs go to a per-lane
+//                  segment list in shared memory.  The loops over dy, dz are
+//                  unrolled for the stencil half-widths 1..3 so that the per-axis
+//                  gaps are computed 2(2W+1) times, not (2W+1)^2 times.
+//   walk phase  -- every lane walks ITS OWN list, kSChunk loads per iteration;
+//                  the warp runs for the longest list, and a list is the sum of
+//                  ~20-60 runs, so the lanes are far better balanced than in a
+//                  lock step over single rows.  The force is evaluated inline
+//                  under the predicate of fp32 contract #2 (a queued force phase
+//                  as in variant 1 was measured slower here: 228 vs 135 us on C3).
+//                  A slot past the end of a run reads the lane's own position,
+//                  which the j != i term of the predicate rejects.
+// Conservative by construction: the bounds are widened by `marg` cells, >= 4x the
+// rounding error of contract #1, and r_c^2 by 2^-10, so no in-range pair is ever
+// dropped; an extra candidate only costs a test.
+constexpr int kSThreads = 128;
+constexpr int kSegCap = 24;       // segments per lane between walks
+constexpr int kSChunk = 4;
+
+template <int N> struct IntC { static constexpr int value = N; };
+
+template <bool kCharged>
+__global__ void __launch_bounds__(kSThreads, 4)
+k_pair_force_s(const __grid_constant__ LvDev P, const float4 *__restrict__ pos,
+               const uint32_t *__restrict__ off, float4 *__restrict__ force)
+{
+    __shared__ LvPair s_pair[LV_MAX_TYPES * LV_MAX_TYPES];
+    __shared__ int8_t s_w[LV_MAX_TYPES * LV_MAX_TYPES];
+    __shared__ uint2 s_seg[kSegCap * kSThreads];
+    if (threadIdx.x < LV_MAX_TYPES * LV_MAX_TYPES) {
+        s_pair[threadIdx.x] = P.pair[threadIdx.x];
+        s_w[threadIdx.x] = P.w[threadIdx.x];
+    }
+    __syncthreads();
+    const int i = P.n - 1 - (int)(blockIdx.x * kSThreads + threadIdx.x);
+    const bool live = i >= 0;
+    const uint32_t self = live ? (uint32_t)i : 0u;
+    const float4 pi = pos[self];
+    const int a = live ? __float_as_int(pi.w) : 0;
+    const LvPair *pair_a = s_pair + a * LV_MAX_TYPES;
+    uint2 *seg = s_seg + threadIdx.x;
+    float fx = 0.f, fy = 0.f, fz = 0.f;
+    int cnt = 0;
+    int nseg = 0;
+
+    float rc2 = 0.f, c12 = 0.f, c6 = 0.f, qq = 0.f;    // pair (a, b) of the grid being walked
+    auto walk = [&]() {
+        int s = 0;
+        uint32_t j = 0u, je = 0u;
+        for (;;) {
+            // the next kSChunk slots of this lane's list, runs joined end to end (no padding
+            // of a run to the chunk); a lane that has run out reads its own position
+            uint32_t jj[kSChunk];
+            float4 pj[kSChunk];
+            bool any_valid = false;
+#pragma unroll
+            for (int u = 0; u < kSChunk; ++u) {
+                if (j >= je && s < nseg) {
+                    const uint2 sg = seg[s * kSThreads];
+                    ++s;
+                    j = sg.x;
+                    je = sg.y;
+                }
+                const bool v = j < je;
+                if (u == 0) any_valid = v;
+                jj[u] = v ? j : self;
+                ++j;
+                pj[u] = __ldg(pos + jj[u]);
+            }
+            if (!__any_sync(kFull, any_valid)) break;
+#pragma unroll
+            for (int u = 0; u < kSChunk; ++u) {
+                const float dx = __fsub_rn(pi.x, pj[u].x);
+                const float dy = __fsub_rn(pi.y, pj[u].y);
+                const float dz = __fsub_rn(pi.z, pj[u].z);
+                const float r2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
+                const bool in = r2 < rc2 && jj[u] != self;           // fp32 contract #2
+                const float rinv = rsqrt_approx(r2);
+                const float ir2 = rinv * rinv;
+                const float ir6 = ir2 * ir2 * ir2;
+                float f = fmaf(c12, ir6, -c6) * ir6;
+                if (kCharged) f = fmaf(qq, rinv, f);
+                f *= ir2;
+                f = in ? f : 0.0f;      // a select: NaN/inf of a rejected slot never propagates
+                fx = fmaf(f, dx, fx);
+                fy = fmaf(f, dy, fy);
+                fz = fmaf(f, dz, fz);
+                cnt += in ? 1 : 0;
+            }
+        }
+        nseg = 0;
+    };
+
+    for (int b = 0; b < P.n_types; ++b) {
+        const LvGridDev g = P.grid[b];
+        const int w = live ? (int)s_w[a * LV_MAX_TYPES + b] : -1;
+        const int W = __reduce_max_sync(kFull, w);
+        if (W < 0) continue;
+        // contract #1 coordinates of the target on grid b, before the floor
+        const float tx = __fmul_rn(__fsub_rn(pi.x, g.lo), g.inv_h);
+        const float ty = __fmul_rn(__fsub_rn(pi.y, g.lo), g.inv_h);
+        const float tz = __fmul_rn(__fsub_rn(pi.z, g.lo), g.inv_h);
+        const int cx = cell_coord(pi.x, g.lo, g.inv_h, g.G);
+        const int cy = cell_coord(pi.y, g.lo, g.inv_h, g.G);
+        const int cz = cell_coord(pi.z, g.lo, g.inv_h, g.G);
+        const int xlo = max(cx - w, 0), xhi = min(cx + w, g.G - 1);
+        // cell units: rounding of contract #1 moves t by < (G + 8) 2^-23; 4x that as margin
+        const float marg = (float)(g.G + 8) * 4.76837158e-7f;
+        const float rct2 = pair_a[b].rc2 * 1.0009765625f * (g.inv_h * g.inv_h);
+        {
+            const LvPair pr = pair_a[b];
+            rc2 = pr.rc2; c12 = pr.c12; c6 = pr.c6; qq = pr.qq;
+        }
+        // squared gap (cell units) between the target and the cells at offset d along one axis;
+        // cells c >= 1 have a true lower edge and cells c <= G-2 a true upper edge (the clamp
+        // only lengthens the two end cells outwards).  Offsets outside the lane's own stencil
+        // or outside the grid get a gap no cut-off reaches.
+        auto gap2 = [&](int d, int c0, float t) {
+            const int c = c0 + d;
+            float gp = d > 0 ? (float)c - t : (d < 0 ? t - (float)(c + 1) : 0.0f);
+            gp = fmaxf(gp - marg, 0.0f);
+            return (abs(d) <= w && (unsigned)c < (unsigned)g.G) ? gp * gp : 3.0e38f;
+        };
+        auto row = [&](int y, int z, float rem) {
+            // rem <= 1e-6 cannot hold an in-range pair: the 2^-10 slack on r_c^2 is >= 1e-3
+            uint32_t js = 0u, je = 0u;
+            if (rem > 1e-6f) {
+                const float xh = fmaf(rem, rsqrt_approx(rem), marg);   // sqrt to 2 ulp, inside marg
+                const int xa = max(xlo, __float2int_rd(tx - xh));
+                const int xb = min(xhi, __float2int_rd(tx + xh));
+                if (xa <= xb) {
+                    const uint32_t r0 = g.base + (uint32_t)((z * g.G + y) * g.G);
+                    js = __ldg(off + r0 + xa);
+                    je = __ldg(off + r0 + xb + 1);
+                }
+            }
+            if (je > js) {
+                seg[nseg * kSThreads] = make_uint2(js, je);
+                ++nseg;
+            }
+        };
+        auto rows = [&](auto Wc) {
+            constexpr int kW = decltype(Wc)::value;
+            float gy2[2 * kW + 1];
+#pragma unroll
+            for (int d = -kW; d <= kW; ++d) gy2[d + kW] = gap2(d, cy, ty);
+#pragma unroll 1
+            for (int dz = -kW; dz <= kW; ++dz) {
+                if (__any_sync(kFull, nseg > kSegCap - (2 * kW + 1))) walk();
+                const float remz = rct2 - gap2(dz, cz, tz);
+#pragma unroll
+                for (int d = -kW; d <= kW; ++d) row(cy + d, cz + dz, remz - gy2[d + kW]);
+            }
+        };
+        if (W == 1) rows(IntC<1>());
+        else if (W == 2) rows(IntC<2>());
+        else if (W == 3) rows(IntC<3>());
+        else {
+            for (int dz = -W; dz <= W; ++dz) {
+                const float remz = rct2 - gap2(dz, cz, tz);
+                for (int dy = -W; dy <= W; ++dy) {
+                    if (__any_sync(kFull, nseg >= kSegCap)) walk();
+                    row(cy + dy, cz + dz, remz - gap2(dy, cy, ty));
+                }
+            }
+        }
+        walk();
+    }
+    if (live) force[i] = make_float4(fx, fy, fz, __int_as_float(cnt));
+}
+
 // ------------------------------------------------- A1 + A7 fused update
 __device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
                                               uint32_t k0, uint32_t k1, uint32_t out[4])
@@ -606,9 +787,19 @@ cudaError_t lvk_pair_force(const LvDev &P, const LvBufs &B, int variant, cudaStr
 {
     if (variant == 0)
         k_pair_force<<<blocks_for(P.n), kThreads, 0, st>>>(P, B.posB, B.cell_off, B.force);
-    else
+    else if (variant == 1)
         k_pair_force_q<<<(P.n + kFThreads - 1) / kFThreads, kFThreads, 0, st>>>(P, B.posB, B.cell_off,
                                                                              B.force);
+    else {
+        bool charged = false;
+        for (int a = 0; a < P.n_types; ++a)
+            for (int b = 0; b < P.n_types; ++b) charged |= P.pair[a * LV_MAX_TYPES + b].qq != 0.0f;
+        const int blocks = (P.n + kSThreads - 1) / kSThreads;
+        if (charged)
+            k_pair_force_s<true><<<blocks, kSThreads, 0, st>>>(P, B.posB, B.cell_off, B.force);
+        else
+            k_pair_force_s<false><<<blocks, kSThreads, 0, st>>>(P, B.posB, B.cell_off, B.force);
+    }
     return cudaGetLastError();
 }
 

@@ -359,7 +359,7 @@ def test_explicit_interaction_matrix(B, orc):
 
 
 VARIANTS = [  # (sort, force kernel): lv_set_option; (0, 1) is the default path
-    (1, 0), (1, 1), (0, 0),
+    (1, 0), (1, 1), (0, 0), (0, 2),
 ]
 
 
