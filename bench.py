@@ -182,8 +182,8 @@ def run_lv(args):
     base = workloads.make_workload(args.workload, state=False)
     w = workloads.make_workload(args.workload, seed=replicas.replica_seed(base.seed, rank))
     options = None if args.force_kernel is None else {binding.OPT_FORCE_KERNEL: args.force_kernel}
-    sim = binding.Simulation.from_workload(w, cells_per_cut=args.cells_per_cut, device=device,
-                                           options=options)
+    cpc = args.cells_per_cut if args.cells_per_cut else w.tuned_cells_per_cut
+    sim = binding.Simulation.from_workload(w, cells_per_cut=cpc, device=device, options=options)
     if args.start_step > 0:
         sim.step(args.start_step)
         sim.get_state()                      # synchronises; raises on a non-finite state
@@ -256,7 +256,7 @@ def run_lv(args):
     peak_tflops = n_sms * FP32_LANES_PER_SM * 2 * pk["sm_max_mhz"] * 1e6 * 1e-12
     achieved = flops / (force_ms * 1e-3) * 1e-12
     roofline = {
-        "kernel": "k_pair_force", "bound": "alu",
+        "kernel": "k_pair_force_s" if args.force_kernel in (None, 2, 3) else "k_pair_force", "bound": "alu",
         "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s",
         "frac": achieved / peak_tflops,
         "traffic": args.force_traffic_bytes,
@@ -277,6 +277,9 @@ def run_lv(args):
         "config": {"workload": f"{w.name} (BASELINE.json configs[{int(w.name[1]) - 1}]): N={n}, "
                                f"{w.n_types} types, steps {args.start_step + 0}.. of the schedule",
                    "n_particles": n, "start_step": args.start_step,
+                   "cells_per_cut": list(cpc) if cpc else [1] * w.n_types,
+                   "force_kernel": {0: "simple", 1: "queued", 2: "segments", 3: "packed"}[
+                       2 if args.force_kernel is None else args.force_kernel],
                    "replicas": world, "parallelism": "independent replicas, no collective",
                    "l2": "flushed between timed steps (256 MiB memset on the same stream)",
                    "timing": "CUDA events on the library's stream around every step; sum over K"},

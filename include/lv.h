@@ -137,11 +137,15 @@ int lv_set_grid(lv_sim *s, const int32_t *cells_per_cut);
  *                        whose single digit is the whole key -- histogram, scan,
  *                        stable scatter (4 kernels); LV_SORT_RADIX: the on-board
  *                        multi-pass LSD radix sort (CUB) + offsets/scatter kernel.
- *   LV_OPT_FORCE_KERNEL  LV_FORCE_QUEUED (default): test phase / force phase with
- *                        per-thread in-range queues; LV_FORCE_SIMPLE: the first
- *                        kernel (inline force), kept as the measured baseline.
- * Both settings of either option give bit-identical permutations, offsets and
- * neighbour counts; forces agree to rounding (identical summation order). */
+ *   LV_OPT_FORCE_KERNEL  LV_FORCE_SEGMENTS (default): ball-trimmed stencil rows kept as
+ *                        per-lane run lists, walked end to end with the force inline;
+ *                        LV_FORCE_PACKED: the same with aligned slot pairs and packed
+ *                        f32x2 arithmetic (faster in dense mixed states, slower in
+ *                        dilute ones); LV_FORCE_QUEUED: row-by-row lock step with
+ *                        per-thread in-range queues; LV_FORCE_SIMPLE: the first kernel.
+ *                        The last two are kept as measured baselines.
+ * Every setting gives bit-identical permutations, offsets and neighbour counts;
+ * forces agree to rounding. */
 #define LV_OPT_SORT          1
 #define LV_OPT_FORCE_KERNEL  2
 #define LV_SORT_COUNTING     0
@@ -149,6 +153,7 @@ int lv_set_grid(lv_sim *s, const int32_t *cells_per_cut);
 #define LV_FORCE_SIMPLE      0
 #define LV_FORCE_QUEUED      1
 #define LV_FORCE_SEGMENTS    2
+#define LV_FORCE_PACKED      3
 int lv_set_option(lv_sim *s, int option, int value);
 
 /* Bytes of device workspace lv_bind needs (0 if types are not set). */

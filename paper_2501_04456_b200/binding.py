@@ -24,7 +24,7 @@ DBG_KEYS, DBG_KEYS_SORTED, DBG_PERM, DBG_CELL_OFFSETS, DBG_IDS_SORTED, DBG_GRID 
 E_NONFINITE = -5
 OPT_SORT, OPT_FORCE_KERNEL = 1, 2
 SORT_COUNTING, SORT_RADIX = 0, 1
-FORCE_SIMPLE, FORCE_QUEUED, FORCE_SEGMENTS = 0, 1, 2
+FORCE_SIMPLE, FORCE_QUEUED, FORCE_SEGMENTS, FORCE_PACKED = 0, 1, 2, 3
 
 # every symbol include/lv.h declares (tests check the library exports them all)
 SYMBOLS = ["lv_langevin_coeffs", "lv_create", "lv_set_types", "lv_set_forces",

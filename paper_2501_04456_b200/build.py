@@ -15,6 +15,7 @@ SOURCES = ["lv_api.cu", "lv_kernels.cu", "lv_sort.cu"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
          "-Xcompiler", "-fPIC", "-I", os.path.join(ROOT, "include"), "-I", CSRC]
+FLAGS += os.environ.get("LV_NVCC_EXTRA", "").split()     # e.g. -DLV_S_CHUNK=2 for tuning sweeps
 
 
 def _deps():

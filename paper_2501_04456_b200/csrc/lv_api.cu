@@ -28,7 +28,7 @@ struct lv_sim {
     int64_t sched_steps = 0;
     int32_t cells_per_cut[LV_MAX_TYPES];
     int sort_mode = LV_SORT_COUNTING;
-    int force_kernel = LV_FORCE_QUEUED;
+    int force_kernel = LV_FORCE_SEGMENTS;
     lv_grid_info grid;
     int sort_end_bit = 1;
     size_t ws_bytes = 0;
@@ -101,7 +101,7 @@ int derive_grid(lv_sim *s)
 
 struct Layout {
     size_t posA, velA, posB, velB, force, key_in, key_out, val_in, val_out, cell_off, sort_temp,
-        sort_temp_bytes, st, staging, cell_cnt, scan_tile, scan_ticket, total;
+        sort_temp_bytes, st, staging, cell_cnt, scan_tile, scan_ticket, posP, total;
 };
 
 Layout layout_of(const lv_sim *s)
@@ -124,6 +124,7 @@ Layout layout_of(const lv_sim *s)
     L.sort_temp = take(L.sort_temp_bytes);
     L.st = take(sizeof(LvDevState));
     L.staging = take(28 * n);
+    L.posP = take(16 * (n + 4));   // pair-interleaved copy of posB + dummy slots (LV_FORCE_PACKED)
     L.total = o;
     return L;
 }
@@ -193,9 +194,9 @@ int enqueue_stage(lv_sim *s, int stage)
     case 2:
         if (counting) {
             LV_CUDA(s, lvk_place(s->dev, s->bufs, s->stream));
-            LV_CUDA(s, lvk_rank_gather(s->dev, s->bufs, s->stream));
+            LV_CUDA(s, lvk_rank_gather(s->dev, s->bufs, s->force_kernel == LV_FORCE_PACKED, s->stream));
         } else {
-            LV_CUDA(s, lvk_bounds_scatter(s->dev, s->bufs, s->stream));
+            LV_CUDA(s, lvk_bounds_scatter(s->dev, s->bufs, s->force_kernel == LV_FORCE_PACKED, s->stream));
         }
         break;
     case 3:
@@ -389,7 +390,7 @@ int lv_set_option(lv_sim *s, int option, int value)
         s->sort_mode = value;
         return LV_OK;
     case LV_OPT_FORCE_KERNEL:
-        if (value < LV_FORCE_SIMPLE || value > LV_FORCE_SEGMENTS) return LV_E_ARG;
+        if (value < LV_FORCE_SIMPLE || value > LV_FORCE_PACKED) return LV_E_ARG;
         s->force_kernel = value;
         return LV_OK;
     default:
@@ -430,6 +431,7 @@ int lv_bind(lv_sim *s, void *workspace_dev, size_t workspace_bytes, void *cuda_s
     B.cell_cnt = (uint32_t *)(w + L.cell_cnt);
     B.scan_tile = (unsigned long long *)(w + L.scan_tile);
     B.scan_ticket = (unsigned int *)(w + L.scan_ticket);
+    B.posP = (float *)(w + L.posP);
     s->ws_bytes = L.total;
     s->stream = (cudaStream_t)cuda_stream;
     derive_tables(s);

@@ -72,6 +72,10 @@ struct LvBufs {
     size_t sort_temp_bytes;
     LvDevState *st;
     unsigned char *staging;  // n * 28 bytes: host<->device state transfers
+    // Pair-interleaved copy of posB for the packed force kernel: slots 2p and 2p+1 share
+    // 32 bytes {x0, x1, y0, y1, z0, z1, w0, w1}; slots n .. 2*ceil(n/2)+1 are dummies far
+    // outside every cut-off.  Written by the gather only when that kernel is selected.
+    float *posP;
 };
 
 // droplet radius after n steps (step (iii)); fp64 on host and device
@@ -89,12 +93,12 @@ constexpr int kScanTile = 4096;   // cells per tile of the cell-count scan
 
 // ---- launch wrappers (lv_kernels.cu) -- all asynchronous on `st` ----------
 cudaError_t lvk_hash(const LvDev &P, const LvBufs &B, cudaStream_t st);
-cudaError_t lvk_bounds_scatter(const LvDev &P, const LvBufs &B, cudaStream_t st);
+cudaError_t lvk_bounds_scatter(const LvDev &P, const LvBufs &B, bool packed, cudaStream_t st);
 // counting sort (one radix digit = the whole key): hash + count, scan, place, rank + gather
 cudaError_t lvk_hash_count(const LvDev &P, const LvBufs &B, cudaStream_t st);
 cudaError_t lvk_scan_cells(const LvDev &P, const LvBufs &B, cudaStream_t st);
 cudaError_t lvk_place(const LvDev &P, const LvBufs &B, cudaStream_t st);
-cudaError_t lvk_rank_gather(const LvDev &P, const LvBufs &B, cudaStream_t st);
+cudaError_t lvk_rank_gather(const LvDev &P, const LvBufs &B, bool packed, cudaStream_t st);
 cudaError_t lvk_keys_sorted(const LvDev &P, const LvBufs &B, uint32_t *out, cudaStream_t st);
 cudaError_t lvk_pair_force(const LvDev &P, const LvBufs &B, int variant, cudaStream_t st);
 cudaError_t lvk_update(const LvDev &P, const LvBufs &B, cudaStream_t st);

@@ -24,6 +24,22 @@ __device__ __forceinline__ int cell_coord(float x, float lo, float inv_h, int G)
     return (int)f;
 }
 
+// Pair-interleaved copy of the cell-sorted positions (LvBufs::posP): slot k goes to
+// floats {x, y, z, w} at 8 (k >> 1) + (k & 1) + {0, 2, 4, 6}.  The thread of the last
+// slot also writes the dummies: slot n if n is odd, and one whole dummy pair after it.
+__device__ __forceinline__ void store_packed(float *posP, int k, int n, float4 p)
+{
+    float *q = posP + 8 * (size_t)(k >> 1) + (k & 1);
+    q[0] = p.x; q[2] = p.y; q[4] = p.z; q[6] = p.w;
+    if (k == n - 1) {
+        const int n_even = (n + 1) & ~1;
+        for (int d = n; d < n_even + 2; ++d) {
+            float *r = posP + 8 * (size_t)(d >> 1) + (d & 1);
+            r[0] = 1e18f; r[2] = 0.f; r[4] = 0.f; r[6] = 0.f;
+        }
+    }
+}
+
 // ---------------------------------------------------------------- A2 hash
 __global__ void __launch_bounds__(kThreads)
 k_hash(const __grid_constant__ LvDev P, const float4 *__restrict__ pos,
@@ -66,7 +82,7 @@ __global__ void __launch_bounds__(kThreads)
 k_bounds_scatter(const __grid_constant__ LvDev P, const uint32_t *__restrict__ key_sorted,
                  const uint32_t *__restrict__ perm, const float4 *__restrict__ posA,
                  const float4 *__restrict__ velA, float4 *__restrict__ posB,
-                 float4 *__restrict__ velB, uint32_t *__restrict__ off)
+                 float4 *__restrict__ velB, uint32_t *__restrict__ off, float *__restrict__ posP)
 {
     int k = blockIdx.x * kThreads + threadIdx.x;
     unsigned lane = threadIdx.x & 31;
@@ -82,8 +98,10 @@ k_bounds_scatter(const __grid_constant__ LvDev P, const uint32_t *__restrict__ k
         }
         if (k == P.n - 1) { tail_first = key + 1; tail_count = P.n_cells - key; }
         uint32_t src = perm[k];
-        posB[k] = posA[src];
+        const float4 p = posA[src];
+        posB[k] = p;
         velB[k] = velA[src];
+        if (posP) store_packed(posP, k, P.n, p);
     }
     warp_fill(off, first, count, (uint32_t)k, lane);
     warp_fill(off, tail_first, tail_count, (uint32_t)P.n, lane);
@@ -215,7 +233,7 @@ __global__ void __launch_bounds__(kThreads)
 k_rank_gather(int n, const uint32_t *__restrict__ key, const uint32_t *__restrict__ off,
               const uint32_t *__restrict__ arrival, uint32_t *__restrict__ perm,
               const float4 *__restrict__ posA, const float4 *__restrict__ velA,
-              float4 *__restrict__ posB, float4 *__restrict__ velB)
+              float4 *__restrict__ posB, float4 *__restrict__ velB, float *__restrict__ posP)
 {
     int k = blockIdx.x * kThreads + threadIdx.x;
     if (k >= n) return;
@@ -229,6 +247,7 @@ k_rank_gather(int n, const uint32_t *__restrict__ key, const uint32_t *__restric
     perm[dst] = v;
     posB[dst] = p;
     velB[dst] = u;
+    if (posP) store_packed(posP, (int)dst, n, p);
 }
 
 __global__ void __launch_bounds__(kThreads)
@@ -474,23 +493,66 @@ k_pair_force_q(const __grid_constant__ LvDev P, const float4 *__restrict__ pos,
 // Conservative by construction: the bounds are widened by `marg` cells, >= 4x the
 // rounding error of contract #1, and r_c^2 by 2^-10, so no in-range pair is ever
 // dropped; an extra candidate only costs a test.
-constexpr int kSThreads = 128;
+#ifndef LV_S_THREADS
+#define LV_S_THREADS 128
+#endif
+#ifndef LV_S_CHUNK
+#define LV_S_CHUNK 4
+#endif
+#ifndef LV_S_MINBLOCKS
+#define LV_S_MINBLOCKS 4
+#endif
+constexpr int kSThreads = LV_S_THREADS;
 constexpr int kSegCap = 24;       // segments per lane between walks
-constexpr int kSChunk = 4;
+constexpr int kSChunk = LV_S_CHUNK;
 
 template <int N> struct IntC { static constexpr int value = N; };
 
-template <bool kCharged>
-__global__ void __launch_bounds__(kSThreads, 4)
+// Two fp32 lanes in one 64-bit register pair (sm_100 FADD2 / FMUL2 / FFMA2): each half is
+// an IEEE round-to-nearest operation, so contract #2 holds per half; one instruction issue
+// serves two candidates.
+typedef unsigned long long f32x2;
+__device__ __forceinline__ f32x2 pack2(float lo, float hi)
+{
+    f32x2 r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ void unpack2(f32x2 v, float &lo, float &hi)
+{
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ f32x2 sub2(f32x2 a, f32x2 b)
+{
+    f32x2 r;
+    asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+__device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b)
+{
+    f32x2 r;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+__device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c)
+{
+    f32x2 r;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
+    return r;
+}
+
+template <bool kCharged, bool kPacked>
+__global__ void __launch_bounds__(kSThreads, LV_S_MINBLOCKS)
 k_pair_force_s(const __grid_constant__ LvDev P, const float4 *__restrict__ pos,
-               const uint32_t *__restrict__ off, float4 *__restrict__ force)
+               const uint32_t *__restrict__ off, float4 *__restrict__ force,
+               const float *__restrict__ posP)
 {
     __shared__ LvPair s_pair[LV_MAX_TYPES * LV_MAX_TYPES];
     __shared__ int8_t s_w[LV_MAX_TYPES * LV_MAX_TYPES];
     __shared__ uint2 s_seg[kSegCap * kSThreads];
-    if (threadIdx.x < LV_MAX_TYPES * LV_MAX_TYPES) {
-        s_pair[threadIdx.x] = P.pair[threadIdx.x];
-        s_w[threadIdx.x] = P.w[threadIdx.x];
+    for (int t = threadIdx.x; t < LV_MAX_TYPES * LV_MAX_TYPES; t += kSThreads) {
+        s_pair[t] = P.pair[t];
+        s_w[t] = P.w[t];
     }
     __syncthreads();
     const int i = P.n - 1 - (int)(blockIdx.x * kSThreads + threadIdx.x);
@@ -505,15 +567,14 @@ k_pair_force_s(const __grid_constant__ LvDev P, const float4 *__restrict__ pos,
     int nseg = 0;
 
     float rc2 = 0.f, c12 = 0.f, c6 = 0.f, qq = 0.f;    // pair (a, b) of the grid being walked
-    auto walk = [&]() {
+    auto walk_scalar = [&]() {
         int s = 0;
         uint32_t j = 0u, je = 0u;
-        for (;;) {
-            // the next kSChunk slots of this lane's list, runs joined end to end (no padding
-            // of a run to the chunk); a lane that has run out reads its own position
-            uint32_t jj[kSChunk];
-            float4 pj[kSChunk];
-            bool any_valid = false;
+        // the next kSChunk slots of this lane's list, runs joined end to end (no padding of
+        // a run to the chunk); a lane that has run out reads its own position.  Returns
+        // whether the lane still had a slot.
+        auto fetch = [&](uint32_t (&jj)[kSChunk], float4 (&pj)[kSChunk]) {
+            bool valid = false;
 #pragma unroll
             for (int u = 0; u < kSChunk; ++u) {
                 if (j >= je && s < nseg) {
@@ -523,12 +584,14 @@ k_pair_force_s(const __grid_constant__ LvDev P, const float4 *__restrict__ pos,
                     je = sg.y;
                 }
                 const bool v = j < je;
-                if (u == 0) any_valid = v;
+                if (u == 0) valid = v;
                 jj[u] = v ? j : self;
                 ++j;
                 pj[u] = __ldg(pos + jj[u]);
             }
-            if (!__any_sync(kFull, any_valid)) break;
+            return valid;
+        };
+        auto eval = [&](const uint32_t (&jj)[kSChunk], const float4 (&pj)[kSChunk]) {
 #pragma unroll
             for (int u = 0; u < kSChunk; ++u) {
                 const float dx = __fsub_rn(pi.x, pj[u].x);
@@ -548,8 +611,101 @@ k_pair_force_s(const __grid_constant__ LvDev P, const float4 *__restrict__ pos,
                 fz = fmaf(f, dz, fz);
                 cnt += in ? 1 : 0;
             }
+        };
+        // two chunks in flight: the loads of one are issued before the other is evaluated
+        uint32_t ja[kSChunk], jb[kSChunk];
+        float4 pa[kSChunk], pb[kSChunk];
+        bool va = fetch(ja, pa);
+        for (;;) {
+            if (!__any_sync(kFull, va)) break;
+            const bool vb = fetch(jb, pb);
+            eval(ja, pa);
+            if (!__any_sync(kFull, vb)) break;
+            va = fetch(ja, pa);
+            eval(jb, pb);
         }
         nseg = 0;
+    };
+
+    // Packed walk (LV_FORCE_PACKED): the lane steps through ALIGNED PAIRS of slots of the
+    // pair-interleaved copy posP -- one 32-byte load {x0,x1,y0,y1,z0,z1,w0,w1} per pair,
+    // FADD2 / FMUL2 / FFMA2 on both halves at once.  A half is valid iff its slot index
+    // lies inside the run, (idx - js) <u (je - js); the lane's own slot never appears in a
+    // run (push splits the run of the own cell around it), so there is no j != i test.
+    // A lane that has run out reads the dummy pair behind the last slot.
+    constexpr int kPairs = kSChunk / 2;
+    f32x2 fx2 = 0ull, fy2 = 0ull, fz2 = 0ull;          // (0.f, 0.f)
+    auto walk_packed = [&]() {
+        int s = 0;
+        uint32_t j = 0u, jb = 0u, je = 0u;
+        const uint32_t dummy = ((uint32_t)P.n + 1u) & ~1u;
+        const f32x2 pix = pack2(pi.x, pi.x), piy = pack2(pi.y, pi.y), piz = pack2(pi.z, pi.z);
+        const f32x2 c12v = pack2(c12, c12), nc6v = pack2(-c6, -c6), qqv = pack2(qq, qq);
+        auto fetch = [&](uint32_t (&rel)[kPairs], uint32_t (&len)[kPairs], f32x2 (&X)[kPairs],
+                         f32x2 (&Y)[kPairs], f32x2 (&Z)[kPairs]) {
+            bool valid = false;
+#pragma unroll
+            for (int u = 0; u < kPairs; ++u) {
+                if (j >= je && s < nseg) {
+                    const uint2 sg = seg[s * kSThreads];
+                    ++s;
+                    jb = sg.x;
+                    je = sg.y;
+                    j = jb & ~1u;
+                }
+                if (u == 0) valid = j < je;
+                rel[u] = j - jb;
+                len[u] = je - jb;
+                const uint32_t ja = j < je ? j : dummy;
+                j += 2u;
+                f32x2 wv;
+                asm("ld.global.nc.v4.b64 {%0, %1, %2, %3}, [%4];"
+                    : "=l"(X[u]), "=l"(Y[u]), "=l"(Z[u]), "=l"(wv)
+                    : "l"(posP + 4 * (size_t)ja));
+            }
+            return valid;
+        };
+        auto eval = [&](const uint32_t (&rel)[kPairs], const uint32_t (&len)[kPairs],
+                        const f32x2 (&X)[kPairs], const f32x2 (&Y)[kPairs], const f32x2 (&Z)[kPairs]) {
+#pragma unroll
+            for (int u = 0; u < kPairs; ++u) {
+                const f32x2 dx = sub2(pix, X[u]), dy = sub2(piy, Y[u]), dz = sub2(piz, Z[u]);
+                const f32x2 r2 = fma2(dz, dz, fma2(dy, dy, mul2(dx, dx)));   // contract #2, per half
+                float r2a, r2b;
+                unpack2(r2, r2a, r2b);
+                const bool in0 = r2a < rc2 && rel[u] < len[u];
+                const bool in1 = r2b < rc2 && rel[u] + 1u < len[u];
+                const f32x2 rinv = pack2(rsqrt_approx(r2a), rsqrt_approx(r2b));
+                const f32x2 ir2 = mul2(rinv, rinv);
+                const f32x2 ir6 = mul2(mul2(ir2, ir2), ir2);
+                f32x2 f = mul2(fma2(c12v, ir6, nc6v), ir6);
+                if (kCharged) f = fma2(qqv, rinv, f);
+                f = mul2(f, ir2);
+                float fa, fb;
+                unpack2(f, fa, fb);
+                f = pack2(in0 ? fa : 0.0f, in1 ? fb : 0.0f);   // selects: a rejected half never propagates
+                fx2 = fma2(f, dx, fx2);
+                fy2 = fma2(f, dy, fy2);
+                fz2 = fma2(f, dz, fz2);
+                cnt += (in0 ? 1 : 0) + (in1 ? 1 : 0);
+            }
+        };
+        uint32_t ra[kPairs], la[kPairs], rb[kPairs], lb[kPairs];
+        f32x2 Xa[kPairs], Ya[kPairs], Za[kPairs], Xb[kPairs], Yb[kPairs], Zb[kPairs];
+        bool va = fetch(ra, la, Xa, Ya, Za);
+        for (;;) {
+            if (!__any_sync(kFull, va)) break;
+            const bool vb = fetch(rb, lb, Xb, Yb, Zb);
+            eval(ra, la, Xa, Ya, Za);
+            if (!__any_sync(kFull, vb)) break;
+            va = fetch(ra, la, Xa, Ya, Za);
+            eval(rb, lb, Xb, Yb, Zb);
+        }
+        nseg = 0;
+    };
+    auto walk = [&]() {
+        if constexpr (kPacked) walk_packed();
+        else walk_scalar();
     };
 
     for (int b = 0; b < P.n_types; ++b) {
@@ -582,18 +738,27 @@ k_pair_force_s(const __grid_constant__ LvDev P, const float4 *__restrict__ pos,
             gp = fmaxf(gp - marg, 0.0f);
             return (abs(d) <= w && (unsigned)c < (unsigned)g.G) ? gp * gp : 3.0e38f;
         };
-        auto row = [&](int y, int z, float rem) {
-            // rem <= 1e-6 cannot hold an in-range pair: the 2^-10 slack on r_c^2 is >= 1e-3
-            uint32_t js = 0u, je = 0u;
-            if (rem > 1e-6f) {
-                const float xh = fmaf(rem, rsqrt_approx(rem), marg);   // sqrt to 2 ulp, inside marg
-                const int xa = max(xlo, __float2int_rd(tx - xh));
-                const int xb = min(xhi, __float2int_rd(tx + xh));
-                if (xa <= xb) {
-                    const uint32_t r0 = g.base + (uint32_t)((z * g.G + y) * g.G);
-                    js = __ldg(off + r0 + xa);
-                    je = __ldg(off + r0 + xb + 1);
+        // bounds of one row, branch-free so that the loads of a whole dz-slab are in flight
+        // together: a row that cannot hold an in-range pair (rem <= 1e-6: the 2^-10 slack on
+        // r_c^2 is >= 1e-3) reads the lane's own cell twice and comes out empty
+        const uint32_t own = g.base + (uint32_t)((cz * g.G + cy) * g.G + cx);
+        auto bounds = [&](int y, int z, float rem, uint32_t &js, uint32_t &je) {
+            const float remp = fmaxf(rem, 1e-6f);
+            const float xh = fmaf(remp, rsqrt_approx(remp), marg);   // sqrt to 2 ulp, inside marg
+            const int xa = max(xlo, __float2int_rd(tx - xh));
+            const int xb = min(xhi, __float2int_rd(tx + xh));
+            const bool ok = rem > 1e-6f && xa <= xb;
+            const uint32_t r0 = g.base + (uint32_t)((z * g.G + y) * g.G);
+            js = __ldg(off + (ok ? r0 + xa : own));
+            je = __ldg(off + (ok ? r0 + xb + 1 : own));
+        };
+        auto push = [&](uint32_t js, uint32_t je) {
+            if (kPacked && live && self - js < je - js) {     // the run of the own cell: cut i out
+                if (self > js) {
+                    seg[nseg * kSThreads] = make_uint2(js, self);
+                    ++nseg;
                 }
+                js = self + 1u;
             }
             if (je > js) {
                 seg[nseg * kSThreads] = make_uint2(js, je);
@@ -607,10 +772,14 @@ k_pair_force_s(const __grid_constant__ LvDev P, const float4 *__restrict__ pos,
             for (int d = -kW; d <= kW; ++d) gy2[d + kW] = gap2(d, cy, ty);
 #pragma unroll 1
             for (int dz = -kW; dz <= kW; ++dz) {
-                if (__any_sync(kFull, nseg > kSegCap - (2 * kW + 1))) walk();
+                if (__any_sync(kFull, nseg > kSegCap - (2 * kW + 2))) walk();
                 const float remz = rct2 - gap2(dz, cz, tz);
+                uint32_t js[2 * kW + 1], je[2 * kW + 1];
 #pragma unroll
-                for (int d = -kW; d <= kW; ++d) row(cy + d, cz + dz, remz - gy2[d + kW]);
+                for (int d = -kW; d <= kW; ++d)
+                    bounds(cy + d, cz + dz, remz - gy2[d + kW], js[d + kW], je[d + kW]);
+#pragma unroll
+                for (int d = -kW; d <= kW; ++d) push(js[d + kW], je[d + kW]);
             }
         };
         if (W == 1) rows(IntC<1>());
@@ -620,12 +789,20 @@ k_pair_force_s(const __grid_constant__ LvDev P, const float4 *__restrict__ pos,
             for (int dz = -W; dz <= W; ++dz) {
                 const float remz = rct2 - gap2(dz, cz, tz);
                 for (int dy = -W; dy <= W; ++dy) {
-                    if (__any_sync(kFull, nseg >= kSegCap)) walk();
-                    row(cy + dy, cz + dz, remz - gap2(dy, cy, ty));
+                    if (__any_sync(kFull, nseg >= kSegCap - 1)) walk();
+                    uint32_t js, je;
+                    bounds(cy + dy, cz + dz, remz - gap2(dy, cy, ty), js, je);
+                    push(js, je);
                 }
             }
         }
         walk();
+    }
+    if (kPacked) {
+        float lo, hi;
+        unpack2(fx2, lo, hi); fx = lo + hi;
+        unpack2(fy2, lo, hi); fy = lo + hi;
+        unpack2(fz2, lo, hi); fz = lo + hi;
     }
     if (live) force[i] = make_float4(fx, fy, fz, __int_as_float(cnt));
 }
@@ -776,10 +953,11 @@ cudaError_t lvk_hash(const LvDev &P, const LvBufs &B, cudaStream_t st)
     return cudaGetLastError();
 }
 
-cudaError_t lvk_bounds_scatter(const LvDev &P, const LvBufs &B, cudaStream_t st)
+cudaError_t lvk_bounds_scatter(const LvDev &P, const LvBufs &B, bool packed, cudaStream_t st)
 {
     k_bounds_scatter<<<blocks_for(P.n), kThreads, 0, st>>>(P, B.key_out, B.val_out, B.posA, B.velA,
-                                                           B.posB, B.velB, B.cell_off);
+                                                           B.posB, B.velB, B.cell_off,
+                                                           packed ? B.posP : nullptr);
     return cudaGetLastError();
 }
 
@@ -795,10 +973,17 @@ cudaError_t lvk_pair_force(const LvDev &P, const LvBufs &B, int variant, cudaStr
         for (int a = 0; a < P.n_types; ++a)
             for (int b = 0; b < P.n_types; ++b) charged |= P.pair[a * LV_MAX_TYPES + b].qq != 0.0f;
         const int blocks = (P.n + kSThreads - 1) / kSThreads;
-        if (charged)
-            k_pair_force_s<true><<<blocks, kSThreads, 0, st>>>(P, B.posB, B.cell_off, B.force);
-        else
-            k_pair_force_s<false><<<blocks, kSThreads, 0, st>>>(P, B.posB, B.cell_off, B.force);
+        if (variant == 3) {
+            if (charged)
+                k_pair_force_s<true, true><<<blocks, kSThreads, 0, st>>>(P, B.posB, B.cell_off, B.force, B.posP);
+            else
+                k_pair_force_s<false, true><<<blocks, kSThreads, 0, st>>>(P, B.posB, B.cell_off, B.force, B.posP);
+        } else {
+            if (charged)
+                k_pair_force_s<true, false><<<blocks, kSThreads, 0, st>>>(P, B.posB, B.cell_off, B.force, nullptr);
+            else
+                k_pair_force_s<false, false><<<blocks, kSThreads, 0, st>>>(P, B.posB, B.cell_off, B.force, nullptr);
+        }
     }
     return cudaGetLastError();
 }
@@ -824,10 +1009,11 @@ cudaError_t lvk_place(const LvDev &P, const LvBufs &B, cudaStream_t st)
     return cudaGetLastError();
 }
 
-cudaError_t lvk_rank_gather(const LvDev &P, const LvBufs &B, cudaStream_t st)
+cudaError_t lvk_rank_gather(const LvDev &P, const LvBufs &B, bool packed, cudaStream_t st)
 {
     k_rank_gather<<<blocks_for(P.n), kThreads, 0, st>>>(P.n, B.key_in, B.cell_off, B.key_out, B.val_out,
-                                                        B.posA, B.velA, B.posB, B.velB);
+                                                        B.posA, B.velA, B.posB, B.velB,
+                                                        packed ? B.posP : nullptr);
     return cudaGetLastError();
 }
 

@@ -98,11 +98,12 @@ def test_forces_and_counts(B, orc, name, n, cpc):
 
 @pytest.mark.parametrize("name", ["C3", "C4", "C5"])
 def test_forces_full_size(B, orc, name):
-    """BASELINE sizes (N = 2.5e5, 2^20), the launch configuration bench.py times."""
+    """BASELINE sizes (N = 2.5e5, 2^20) in the launch configuration bench.py times
+    (default force kernel, the workload's tuned cells_per_cut)."""
     w = workload(name, None)
     p = orc.params_from_workload(w)
     Fo, So, co, _ = orc.pair_forces(p, w.pos, w.type, "cells")
-    sim = B.Simulation.from_workload(w)
+    sim = B.Simulation.from_workload(w, cells_per_cut=w.tuned_cells_per_cut)
     sim.compute_forces()
     Fg, cg = sim.get_forces()
     assert np.array_equal(cg, co)
@@ -358,8 +359,8 @@ def test_explicit_interaction_matrix(B, orc):
     sim.close()
 
 
-VARIANTS = [  # (sort, force kernel): lv_set_option; (0, 1) is the default path
-    (1, 0), (1, 1), (0, 0), (0, 2),
+VARIANTS = [  # (sort, force kernel): lv_set_option; (0, 2) is the default path
+    (1, 0), (1, 1), (1, 2), (0, 0), (0, 1), (0, 3), (1, 3),
 ]
 
 
@@ -367,7 +368,7 @@ VARIANTS = [  # (sort, force kernel): lv_set_option; (0, 1) is the default path
                                          ("C4", 19999, [2]), ("C2", 8191, None)])
 def test_implementation_options_do_not_change_results(B, orc, name, n, cpc):
     """lv_set_option: the multi-pass radix sort vs the one-digit (counting) sort
-    and the two force kernels give bit-identical cell structures and neighbour
+    and the four force kernels give bit-identical cell structures and neighbour
     counts, forces equal to rounding, and -- for the two sorts -- bit-identical
     trajectories."""
     w = workload(name, n)
@@ -397,7 +398,7 @@ def test_implementation_options_do_not_change_results(B, orc, name, n, cpc):
         sim.step(30)
         x, v, _, _, st = sim.get_state()
         assert st == 30
-        if fk == 1:          # same force kernel as the default: the sort must not matter at all
+        if fk == 2:          # same force kernel as the default: the sort must not matter at all
             assert np.array_equal(x, x0) and np.array_equal(v, v0)
             assert np.array_equal(sim.get_debug(B.DBG_IDS_SORTED), ids0)
         else:
