@@ -61,7 +61,10 @@ extern "C" {
 #define LV_ST_NONFINITE    1u   /* error: also returned as LV_E_NONFINITE */
 #define LV_ST_OUTSIDE_GRID 2u   /* warning: an NP was clamped into a border cell (R22) */
 
-/* lv_get_debug selectors (parity tests) */
+/* lv_get_debug selectors (parity tests).  The views describe the cell rebuild of the last
+ * lv_compute_forces; after lv_step the update kernel has already hashed the NEW positions
+ * for the next step (keys, histogram), so only LV_DBG_IDS_SORTED and LV_DBG_GRID are
+ * meaningful then. */
 #define LV_DBG_KEYS          1  /* uint32[N]   cell key per slot before the sort            */
 #define LV_DBG_KEYS_SORTED   2  /* uint32[N]                                                */
 #define LV_DBG_PERM          3  /* uint32[N]   sorted slot k came from slot perm[k]         */

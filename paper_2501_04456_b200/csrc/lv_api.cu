@@ -15,6 +15,9 @@ struct lv_sim {
     uint64_t seed = 0;
     double dt = 0.0;
     bool types_set = false, sched_set = false, bound = false, state_set = false;
+    // counting mode: keys, arrival ranks and the cell histogram of the CURRENT posA are in
+    // place (written by lv_set_state's first step or by the previous step's update kernel)
+    bool hashed = false;
     lv_type types[LV_MAX_TYPES];
     double eps[LV_MAX_TYPES * LV_MAX_TYPES];
     double sig[LV_MAX_TYPES * LV_MAX_TYPES];
@@ -182,11 +185,16 @@ int enqueue_stage(lv_sim *s, int stage)
     const bool counting = s->sort_mode == LV_SORT_COUNTING;
     switch (stage) {
     case 0:
-        if (counting) LV_CUDA(s, lvk_hash_count(s->dev, s->bufs, s->stream));
-        else LV_CUDA(s, lvk_hash(s->dev, s->bufs, s->stream));
+        if (counting) {
+            // steady state: the previous step's update kernel has already hashed posA
+            if (!s->hashed) LV_CUDA(s, lvk_hash_count(s->dev, s->bufs, s->stream));
+            s->hashed = true;
+        } else {
+            LV_CUDA(s, lvk_hash(s->dev, s->bufs, s->stream));
+        }
         break;
     case 1:
-        if (counting) LV_CUDA(s, lvk_scan_cells(s->dev, s->bufs, s->stream));
+        if (counting) { LV_CUDA(s, lvk_scan_cells(s->dev, s->bufs, s->stream)); s->hashed = false; }
         else LV_CUDA(s, lvs_sort_pairs(s->bufs.sort_temp, s->bufs.sort_temp_bytes, s->bufs.key_in,
                                        s->bufs.key_out, s->bufs.val_in, s->bufs.val_out, s->n,
                                        s->sort_end_bit, s->stream));
@@ -203,7 +211,8 @@ int enqueue_stage(lv_sim *s, int stage)
         LV_CUDA(s, lvk_pair_force(s->dev, s->bufs, s->force_kernel, s->stream));
         break;
     default:
-        LV_CUDA(s, lvk_update(s->dev, s->bufs, s->stream));
+        LV_CUDA(s, lvk_update(s->dev, s->bufs, counting, s->stream));
+        s->hashed = counting;
         break;
     }
     return LV_OK;
@@ -255,7 +264,9 @@ int build_graph(lv_sim *s)
 {
     if (s->stream == nullptr || s->n == 0) return LV_OK;   // legacy stream: direct launches
     LV_CUDA(s, cudaStreamBeginCapture(s->stream, cudaStreamCaptureModeRelaxed));
+    s->hashed = s->sort_mode == LV_SORT_COUNTING;    // the graph is the steady-state step
     int rc = enqueue_step(s);
+    s->hashed = false;
     cudaGraph_t g = nullptr;
     cudaError_t e = cudaStreamEndCapture(s->stream, &g);
     if (rc != LV_OK) { if (g) cudaGraphDestroy(g); return rc; }
@@ -463,6 +474,11 @@ int lv_set_state(lv_sim *s, const float *pos_xyz, const float *vel_xyz, const in
         dt = (const int32_t *)(stg + 24 * n);
     }
     LV_CUDA(s, lvk_pack_state(s->dev, s->bufs, dp, dv, dt, (long long)step, s->stream));
+    if (s->hashed) {     // a histogram of the replaced state is pending: clear it
+        LV_CUDA(s, cudaMemsetAsync(s->bufs.cell_cnt, 0, 4 * ((size_t)s->grid.base[s->n_types] + 1),
+                                   s->stream));
+        s->hashed = false;
+    }
     if (!on_device) LV_CUDA(s, cudaStreamSynchronize(s->stream));
     s->state_set = true;
     return LV_OK;
@@ -484,6 +500,10 @@ int lv_step(lv_sim *s, int n)
     }
     for (int k = 0; k < n; ++k) {
         if (s->graph_exec) {
+            if (s->sort_mode == LV_SORT_COUNTING && !s->hashed) {
+                LV_CUDA(s, lvk_hash_count(s->dev, s->bufs, s->stream));
+                s->hashed = true;        // and the graph's update kernel leaves it true
+            }
             LV_CUDA(s, cudaGraphLaunch(s->graph_exec, s->stream));
         } else {
             int rc = enqueue_step(s);

@@ -101,7 +101,8 @@ cudaError_t lvk_place(const LvDev &P, const LvBufs &B, cudaStream_t st);
 cudaError_t lvk_rank_gather(const LvDev &P, const LvBufs &B, bool packed, cudaStream_t st);
 cudaError_t lvk_keys_sorted(const LvDev &P, const LvBufs &B, uint32_t *out, cudaStream_t st);
 cudaError_t lvk_pair_force(const LvDev &P, const LvBufs &B, int variant, cudaStream_t st);
-cudaError_t lvk_update(const LvDev &P, const LvBufs &B, cudaStream_t st);
+// hash_next: also hash + histogram the new positions for the next step's counting sort
+cudaError_t lvk_update(const LvDev &P, const LvBufs &B, bool hash_next, cudaStream_t st);
 cudaError_t lvk_pack_state(const LvDev &P, const LvBufs &B, const float *pos, const float *vel,
                            const int32_t *type, long long step, cudaStream_t st);
 cudaError_t lvk_unpack_state(const LvDev &P, const LvBufs &B, float *pos, float *vel,

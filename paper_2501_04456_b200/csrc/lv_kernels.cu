@@ -192,19 +192,33 @@ k_scan_cells(uint32_t n_items, uint32_t *__restrict__ cnt, uint32_t *__restrict_
         if (k < (int)wid) wbase += t;
         total += t;
     }
-    if (threadIdx.x == 0) {
+    // look-back by the first warp, 32 predecessors per round (lane 0 = nearest): the
+    // window sums aggregates up to and including the nearest inclusive prefix
+    if (wid == 0) {
         uint32_t excl = 0;
         if (tile > 0) {
-            scan_tile[tile] = (1ull << 32) | total;
-            for (int p = (int)tile - 1; p >= 0; --p) {
-                unsigned long long w;
-                do { w = scan_tile[p]; } while ((w >> 32) == 0ull);
-                excl += (uint32_t)w;
-                if ((w >> 32) == 2ull) break;
+            if (lane == 0) scan_tile[tile] = (1ull << 32) | total;
+            int base = (int)tile - 1;
+            for (;;) {
+                const int p = base - (int)lane;
+                unsigned long long w = 2ull << 32;        // before tile 0: prefix 0
+                if (p >= 0) {
+                    do { w = scan_tile[p]; } while ((w >> 32) == 0ull);
+                }
+                const unsigned incl = __ballot_sync(0xffffffffu, (w >> 32) == 2ull);
+                const int stop = incl ? __ffs(incl) - 1 : 31;     // nearest inclusive prefix
+                uint32_t v = (int)lane <= stop ? (uint32_t)w : 0u;
+#pragma unroll
+                for (int d = 16; d > 0; d >>= 1) v += __shfl_xor_sync(0xffffffffu, v, d);
+                excl += v;
+                if (incl) break;
+                base -= 32;
             }
         }
-        scan_tile[tile] = (2ull << 32) | (unsigned long long)(excl + total);
-        s_excl = excl;
+        if (lane == 0) {
+            scan_tile[tile] = (2ull << 32) | (unsigned long long)(excl + total);
+            s_excl = excl;
+        }
     }
     __syncthreads();
     const uint32_t tbase = s_excl + wbase + (inc - sum);
@@ -828,12 +842,21 @@ __device__ __forceinline__ float u01(uint32_t w)
     return ((float)(w >> 9) + 0.5f) * (1.0f / 8388608.0f);   // exact in fp32, in (0, 1)
 }
 
+// kHash: also do A2 + the histogram of the NEXT step's counting sort on the new position
+// (k_hash_count's work, same fp32 contract #1), so a steady-state step has no hash kernel.
+template <bool kHash>
 __global__ void __launch_bounds__(kThreads)
 k_update(const __grid_constant__ LvDev P, const float4 *__restrict__ posB,
          const float4 *__restrict__ velB, const float4 *__restrict__ force,
-         float4 *__restrict__ posA, float4 *__restrict__ velA, LvDevState *st)
+         float4 *__restrict__ posA, float4 *__restrict__ velA, LvDevState *st,
+         uint32_t *__restrict__ key, uint32_t *__restrict__ rank, uint32_t *__restrict__ cnt,
+         unsigned long long *__restrict__ scan_tile, unsigned int *__restrict__ scan_ticket)
 {
     int i = blockIdx.x * kThreads + threadIdx.x;
+    if (kHash) {
+        if (i < (int)P.n_scan_tiles) scan_tile[i] = 0ull;   // re-arm the next step's scan
+        if (i == 0) *scan_ticket = 0u;
+    }
     const long long n = st->step;                      // index of this step
     __syncthreads();
     // the block that takes the last ticket has seen every block read `step`
@@ -896,6 +919,18 @@ k_update(const __grid_constant__ LvDev P, const float4 *__restrict__ posB,
     velA[i] = make_float4(vx, vy, vz, v.w);
     const float chk = (x + y + z) + (vx + vy + vz);
     if (!(fabsf(chk) <= 3.0e38f)) atomicOr(&st->status, LV_ST_NONFINITE);
+    if (kHash) {
+        const LvGridDev g = P.grid[a];
+        const int cx = cell_coord(x, g.lo, g.inv_h, g.G);
+        const int cy = cell_coord(y, g.lo, g.inv_h, g.G);
+        const int cz = cell_coord(z, g.lo, g.inv_h, g.G);
+        const uint32_t k = g.base + (uint32_t)((cz * g.G + cy) * g.G + cx);
+        key[i] = k;
+        rank[i] = atomicAdd(cnt + k, 1u);
+        const float hi = -g.lo;
+        const bool outside = !(x >= g.lo && x < hi && y >= g.lo && y < hi && z >= g.lo && z < hi);
+        if (outside) atomicOr(&st->status, LV_ST_OUTSIDE_GRID);
+    }
 }
 
 // ------------------------------------------------- state in / out (by id)
@@ -1023,9 +1058,18 @@ cudaError_t lvk_keys_sorted(const LvDev &P, const LvBufs &B, uint32_t *out, cuda
     return cudaGetLastError();
 }
 
-cudaError_t lvk_update(const LvDev &P, const LvBufs &B, cudaStream_t st)
+cudaError_t lvk_update(const LvDev &P, const LvBufs &B, bool hash_next, cudaStream_t st)
 {
-    k_update<<<blocks_for(P.n), kThreads, 0, st>>>(P, B.posB, B.velB, B.force, B.posA, B.velA, B.st);
+    if (hash_next) {
+        const int m = P.n > (int)P.n_scan_tiles ? P.n : (int)P.n_scan_tiles;
+        k_update<true><<<blocks_for(m), kThreads, 0, st>>>(P, B.posB, B.velB, B.force, B.posA, B.velA,
+                                                           B.st, B.key_in, B.val_in, B.cell_cnt,
+                                                           B.scan_tile, B.scan_ticket);
+    } else {
+        k_update<false><<<blocks_for(P.n), kThreads, 0, st>>>(P, B.posB, B.velB, B.force, B.posA,
+                                                            B.velA, B.st, nullptr, nullptr, nullptr,
+                                                            nullptr, nullptr);
+    }
     return cudaGetLastError();
 }
 
