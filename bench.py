@@ -183,7 +183,9 @@ def run_lv(args):
     w = workloads.make_workload(args.workload, seed=replicas.replica_seed(base.seed, rank))
     options = None if args.force_kernel is None else {binding.OPT_FORCE_KERNEL: args.force_kernel}
     cpc = args.cells_per_cut if args.cells_per_cut else w.tuned_cells_per_cut
-    sim = binding.Simulation.from_workload(w, cells_per_cut=cpc, device=device, options=options)
+    nl = None if args.neighbour_list is None else (args.neighbour_list[0], int(args.neighbour_list[1]))
+    sim = binding.Simulation.from_workload(w, cells_per_cut=cpc, device=device, options=options,
+                                           neighbour_list=nl)
     if args.start_step > 0:
         sim.step(args.start_step)
         sim.get_state()                      # synchronises; raises on a non-finite state
@@ -220,6 +222,42 @@ def run_lv(args):
     e1.synchronize()
     res_ms = e0.elapsed_time(e1)
     res_max, _ = replicas.reduce_timing(res_ms, 0.0, device=device)
+
+    # ---- variant (not the headline): persistent skin neighbour list, NEXT-3 -
+    variants = {}
+    if (rank == 0 and world == 1 and nl is None and not args.no_variants
+            and w.tuned_neighbour_list is not None):
+        skin, cap = float(w.tuned_neighbour_list[0]), int(w.tuned_neighbour_list[1])
+        vs = binding.Simulation.from_workload(w, cells_per_cut=cpc, device=device,
+                                              neighbour_list=(skin, cap))
+        if args.start_step > 0:
+            vs.step(args.start_step)
+        timed_steps(vs, torch, flush, max(args.warmup, 3))
+        r0 = vs.rebuild_count()
+        vstages, vtot = timed_steps(vs, torch, flush, args.steps)
+        r1 = vs.rebuild_count()
+        vs.step(max(args.warmup, 3))
+        vs.synchronize()
+        e0.record(vs.stream)
+        vs.step(args.steps)
+        e1.record(vs.stream)
+        e1.synchronize()
+        vres = e0.elapsed_time(e1)
+        vs.get_state()                       # raises if the list overflowed
+        variants["skin_list"] = {
+            "what": "lv_set_neighbour_list: cells + list rebuilt on the device only when an NP has "
+                    "moved skin/2; same neighbour counts, forces to rounding (tests/test_gpu_neighbour_list.py)",
+            "skin": skin, "capacity": cap,
+            "value": float(w.n) * args.steps / (vtot * 1e-3), "unit": UNIT,
+            "ms_per_step": vtot / args.steps,
+            "stage_ms_per_step": {k: v / args.steps for k, v in vstages.items()},
+            "rebuilds_in_timed_region": r1 - r0,
+            "resident_ms_per_step": vres / args.steps,
+            "pair_force_roofline_frac": FLOP_PER_PAIR * 0.5 * (pairs0 + pairs1)
+            / (vstages["pair_force"] / args.steps * 1e-3) * 1e-12
+            / (n_sms * FP32_LANES_PER_SM * 2 * pk["sm_max_mhz"] * 1e6 * 1e-12),
+        }
+        vs.close()
 
     # ---- e2e: host buffers through the C ABI, copies inside the timed region
     n = w.n
@@ -289,6 +327,7 @@ def run_lv(args):
         "stage_ms_per_step": {k: v / args.steps for k, v in stages.items()},
         "wall_s_timed_region": wall_s,
         "roofline": roofline,
+        "variants": variants,
         "resident": {"value": float(n) * args.steps * world / (res_max * 1e-3), "unit": UNIT,
                      "ms_per_step": res_max / args.steps,
                      "how": "lv_step(K) as CUDA-graph replay, no L2 flush, events around the K steps"},
@@ -403,6 +442,9 @@ def main():
     ap.add_argument("--cells-per-cut", type=int, nargs="*", default=None)
     ap.add_argument("--force-kernel", type=int, default=None,
                     help="lv_set_option(LV_OPT_FORCE_KERNEL): 0 simple, 1 queued, 2 segments")
+    ap.add_argument("--neighbour-list", type=float, nargs=2, default=None, metavar=("SKIN", "CAP"),
+                    help="lv_set_neighbour_list: time the skin-list variant instead of the per-step rebuild")
+    ap.add_argument("--no-variants", action="store_true", help="skip the skin-list variant")
     ap.add_argument("--e2e-steps", type=int, default=0)
     ap.add_argument("--snapshots", type=int, nargs="*", default=[10000, 17000])
     ap.add_argument("--snapshot-steps", type=int, default=100)

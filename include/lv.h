@@ -47,6 +47,7 @@ extern "C" {
 #define LV_E_CUDA       -4   /* a CUDA runtime call failed; see lv_last_cuda_error */
 #define LV_E_NONFINITE  -5   /* sticky: a non-finite position or velocity appeared (R6) */
 #define LV_E_NOMEM      -6   /* host allocation failed */
+#define LV_E_CAPACITY   -7   /* sticky: the skin neighbour list overflowed (LV_ST_LIST_OVERFLOW) */
 
 /* droplet schedule modes: step (iii); radius-square law PAPER.md:58 */
 #define LV_SCHED_CONST   0
@@ -60,6 +61,7 @@ extern "C" {
 /* status bits (lv_get_status); warnings do not stop the simulation */
 #define LV_ST_NONFINITE    1u   /* error: also returned as LV_E_NONFINITE */
 #define LV_ST_OUTSIDE_GRID 2u   /* warning: an NP was clamped into a border cell (R22) */
+#define LV_ST_LIST_OVERFLOW 4u  /* error: an NP has more neighbours than the list capacity */
 
 /* lv_get_debug selectors (parity tests).  The views describe the cell rebuild of the last
  * lv_compute_forces; after lv_step the update kernel has already hashed the NEW positions
@@ -158,6 +160,24 @@ int lv_set_grid(lv_sim *s, const int32_t *cells_per_cut);
 #define LV_FORCE_SEGMENTS    2
 #define LV_FORCE_PACKED      3
 int lv_set_option(lv_sim *s, int option, int value);
+
+/* Optional throughput variant: a persistent "skin" neighbour
+ * list.  The paper rebuilds the cells every step only "to identify which [NPs] are close
+ * to each other and can interact"; with capacity > 0 lv_step keeps, per NP,
+ * the slots of every NP within r_c,ab + skin at the last rebuild, evaluates the pair force
+ * from that list (same fp32 contract #2, so the neighbour counts stay bit-identical and
+ * the forces agree to rounding), and rebuilds cells + list on the device -- no host
+ * round trip -- at the first step after any NP has moved farther than skin/2 from where it
+ * was at the build.  skin: length units, > 0.  capacity: list entries per NP (the
+ * workspace grows by 4 * capacity bytes per NP); if an NP has more neighbours the sticky
+ * LV_ST_LIST_OVERFLOW is set and lv_get_state returns LV_E_CAPACITY.  capacity = 0
+ * (default) switches the variant off: every step rebuilds, as the paper does.  Needs
+ * LV_SORT_COUNTING.  lv_compute_forces always uses the cells. */
+int lv_set_neighbour_list(lv_sim *s, double skin, int capacity);
+
+/* Cell/list rebuilds since lv_set_state (host int64, written); counts only steps taken
+ * with the neighbour list on.  Synchronises. */
+int lv_get_rebuild_count(lv_sim *s, int64_t *rebuilds);
 
 /* Bytes of device workspace lv_bind needs (0 if types are not set). */
 size_t lv_workspace_bytes(const lv_sim *s);

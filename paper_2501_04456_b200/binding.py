@@ -19,16 +19,18 @@ from . import build as _build
 MAX_TYPES = 8
 SCHED_CONST, SCHED_LINEAR, SCHED_R2LAW = 0, 1, 2
 WALL_ONESIDED, WALL_WINDOW = 0, 1
-ST_NONFINITE, ST_OUTSIDE_GRID = 1, 2
+ST_NONFINITE, ST_OUTSIDE_GRID, ST_LIST_OVERFLOW = 1, 2, 4
 DBG_KEYS, DBG_KEYS_SORTED, DBG_PERM, DBG_CELL_OFFSETS, DBG_IDS_SORTED, DBG_GRID = 1, 2, 3, 4, 5, 6
 E_NONFINITE = -5
+E_CAPACITY = -7
 OPT_SORT, OPT_FORCE_KERNEL = 1, 2
 SORT_COUNTING, SORT_RADIX = 0, 1
 FORCE_SIMPLE, FORCE_QUEUED, FORCE_SEGMENTS, FORCE_PACKED = 0, 1, 2, 3
 
 # every symbol include/lv.h declares (tests check the library exports them all)
 SYMBOLS = ["lv_langevin_coeffs", "lv_create", "lv_set_types", "lv_set_forces",
-           "lv_set_droplet_schedule", "lv_set_grid", "lv_set_option", "lv_workspace_bytes", "lv_bind",
+           "lv_set_droplet_schedule", "lv_set_grid", "lv_set_option", "lv_set_neighbour_list",
+           "lv_get_rebuild_count", "lv_workspace_bytes", "lv_bind",
            "lv_set_state", "lv_step", "lv_compute_forces", "lv_get_state", "lv_get_forces",
            "lv_get_status", "lv_get_debug", "lv_launches_per_step", "lv_step_profiled",
            "lv_stage_timing", "lv_read_stage_timing",
@@ -73,6 +75,8 @@ def load():
     L.lv_set_droplet_schedule.argtypes = [vp, C.c_int, C.c_double, C.c_double, C.c_int64]
     L.lv_set_grid.argtypes = [vp, ip]
     L.lv_set_option.argtypes = [vp, C.c_int, C.c_int]
+    L.lv_set_neighbour_list.argtypes = [vp, C.c_double, C.c_int]
+    L.lv_get_rebuild_count.argtypes = [vp, C.POINTER(C.c_int64)]
     L.lv_workspace_bytes.argtypes = [vp]
     L.lv_workspace_bytes.restype = C.c_size_t
     L.lv_bind.argtypes = [vp, vp, C.c_size_t, vp]
@@ -160,6 +164,15 @@ class Simulation:
 
     def set_option(self, option: int, value: int):
         self._check(self.L.lv_set_option(self.h, int(option), int(value)), "lv_set_option")
+
+    def set_neighbour_list(self, skin: float, capacity: int):
+        self._check(self.L.lv_set_neighbour_list(self.h, float(skin), int(capacity)),
+                    "lv_set_neighbour_list")
+
+    def rebuild_count(self) -> int:
+        r = C.c_int64()
+        self._check(self.L.lv_get_rebuild_count(self.h, C.byref(r)), "lv_get_rebuild_count")
+        return int(r.value)
 
     def workspace_bytes(self) -> int:
         return int(self.L.lv_workspace_bytes(self.h))
@@ -309,7 +322,7 @@ class Simulation:
     # -- convenience -----------------------------------------------------------
     @classmethod
     def from_workload(cls, w, cells_per_cut=None, device="cuda:0", load_state=True,
-                      options=None) -> "Simulation":
+                      options=None, neighbour_list=None) -> "Simulation":
         """Configure from a workloads.Workload: per-type (a, b) through
         lv_langevin_coeffs, Lorentz-Berthelot tables inside lv_set_types."""
         sim = cls(w.n, w.n_types, w.seed, w.dt, device=device)
@@ -325,6 +338,8 @@ class Simulation:
             sim.set_grid(cells_per_cut)
         for opt, val in (options or {}).items():
             sim.set_option(opt, val)
+        if neighbour_list is not None:          # (skin, capacity)
+            sim.set_neighbour_list(*neighbour_list)
         sim.bind()
         if load_state:
             sim.set_state(w.pos, w.vel, w.type, 0)

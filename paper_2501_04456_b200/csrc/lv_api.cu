@@ -18,6 +18,11 @@ struct lv_sim {
     // counting mode: keys, arrival ranks and the cell histogram of the CURRENT posA are in
     // place (written by lv_set_state's first step or by the previous step's update kernel)
     bool hashed = false;
+    // skin neighbour list (lv_set_neighbour_list); list_cap = 0: off
+    double skin = 0.0;
+    int list_cap = 0;
+    // slot order of `force`: B (ids in velB) after lv_compute_forces, A after lv_step
+    bool force_order_b = true;
     lv_type types[LV_MAX_TYPES];
     double eps[LV_MAX_TYPES * LV_MAX_TYPES];
     double sig[LV_MAX_TYPES * LV_MAX_TYPES];
@@ -104,7 +109,8 @@ int derive_grid(lv_sim *s)
 
 struct Layout {
     size_t posA, velA, posB, velB, force, key_in, key_out, val_in, val_out, cell_off, sort_temp,
-        sort_temp_bytes, st, staging, cell_cnt, scan_tile, scan_ticket, posP, total;
+        sort_temp_bytes, st, staging, cell_cnt, scan_tile, scan_ticket, posP, list, list_rows,
+        pos_ref, total;
 };
 
 Layout layout_of(const lv_sim *s)
@@ -128,6 +134,10 @@ Layout layout_of(const lv_sim *s)
     L.st = take(sizeof(LvDevState));
     L.staging = take(28 * n);
     L.posP = take(16 * (n + 4));   // pair-interleaved copy of posB + dummy slots (LV_FORCE_PACKED)
+    const size_t n_warps = ((n + 127) / 128) * 4;      // warps of the 128-thread force launches
+    L.list = take(s->list_cap > 0 ? 4 * n_warps * 32 * (size_t)s->list_cap : 0);
+    L.list_rows = take(s->list_cap > 0 ? 4 * n_warps : 0);
+    L.pos_ref = take(s->list_cap > 0 ? 16 * n : 0);
     L.total = o;
     return L;
 }
@@ -142,6 +152,12 @@ void derive_tables(lv_sim *s)
     d.n_cells = s->grid.base[T];
     d.n_scan_tiles = (uint32_t)(((size_t)d.n_cells + 1 + kScanTile - 1) / kScanTile);
     d.wall_mode = s->wall_mode;
+    d.list_cap = s->list_cap;
+    d.skin = (float)s->skin;
+    {   // rebuild once an NP is farther than half the skin (less 0.1 % for fp32 rounding) from its build position
+        const double hs = 0.5 * s->skin * (1.0 - 1e-3);
+        d.half_skin2 = (float)(hs * hs);
+    }
     for (int a = 0; a < T; ++a)
         for (int b = 0; b < T; ++b) {
             const int k = a * LV_MAX_TYPES + b;
@@ -151,6 +167,7 @@ void derive_tables(lv_sim *s)
             d.pair[k].c6 = (float)(24.0 * s->eps[k] * s6);
             d.pair[k].qq = (float)(s->coulomb_k * s->types[a].charge * s->types[b].charge);
             d.w[k] = (int8_t)s->grid.w[k];
+            d.wl[k] = (int8_t)std::ceil((s->rcut[k] + s->skin) * (1.0 + 1.0 / 1024.0) / s->grid.h[b]);
         }
     for (int a = 0; a < T; ++a) {
         const lv_type &t = s->types[a];
@@ -180,29 +197,46 @@ void derive_tables(lv_sim *s)
 // The stages of one step, in order (LV_N_STAGES = 5).  Radix mode: hash | CUB radix
 // sort | offsets + scatter | pair force | update.  Counting mode (default): hash +
 // histogram | scan (= cell offsets) | place + rank/gather | pair force | update.
-int enqueue_stage(lv_sim *s, int stage)
+int enqueue_stage(lv_sim *s, int stage, bool list_step = false)
 {
     const bool counting = s->sort_mode == LV_SORT_COUNTING;
+    if (list_step) {
+        // Skin-list step (lv_set_neighbour_list; counting sort only).  Stages 0-2 are the same
+        // rebuild kernels, each returning at once unless the device-side flag of this step is
+        // raised, plus the list build; stages 3-4 work in the list's slot order.
+        switch (stage) {
+        case 0: LV_CUDA(s, lvk_hash_count(s->dev, s->bufs, true, s->stream)); break;
+        case 1: LV_CUDA(s, lvk_scan_cells(s->dev, s->bufs, true, s->stream)); break;
+        case 2:
+            LV_CUDA(s, lvk_place(s->dev, s->bufs, true, s->stream));
+            LV_CUDA(s, lvk_rank_gather(s->dev, s->bufs, false, true, s->stream));
+            LV_CUDA(s, lvk_list_build(s->dev, s->bufs, s->stream));
+            break;
+        case 3: LV_CUDA(s, lvk_pair_force_list(s->dev, s->bufs, s->stream)); break;
+        default: LV_CUDA(s, lvk_update_list(s->dev, s->bufs, s->stream)); break;
+        }
+        return LV_OK;
+    }
     switch (stage) {
     case 0:
         if (counting) {
             // steady state: the previous step's update kernel has already hashed posA
-            if (!s->hashed) LV_CUDA(s, lvk_hash_count(s->dev, s->bufs, s->stream));
+            if (!s->hashed) LV_CUDA(s, lvk_hash_count(s->dev, s->bufs, false, s->stream));
             s->hashed = true;
         } else {
             LV_CUDA(s, lvk_hash(s->dev, s->bufs, s->stream));
         }
         break;
     case 1:
-        if (counting) { LV_CUDA(s, lvk_scan_cells(s->dev, s->bufs, s->stream)); s->hashed = false; }
+        if (counting) { LV_CUDA(s, lvk_scan_cells(s->dev, s->bufs, false, s->stream)); s->hashed = false; }
         else LV_CUDA(s, lvs_sort_pairs(s->bufs.sort_temp, s->bufs.sort_temp_bytes, s->bufs.key_in,
                                        s->bufs.key_out, s->bufs.val_in, s->bufs.val_out, s->n,
                                        s->sort_end_bit, s->stream));
         break;
     case 2:
         if (counting) {
-            LV_CUDA(s, lvk_place(s->dev, s->bufs, s->stream));
-            LV_CUDA(s, lvk_rank_gather(s->dev, s->bufs, s->force_kernel == LV_FORCE_PACKED, s->stream));
+            LV_CUDA(s, lvk_place(s->dev, s->bufs, false, s->stream));
+            LV_CUDA(s, lvk_rank_gather(s->dev, s->bufs, s->force_kernel == LV_FORCE_PACKED, false, s->stream));
         } else {
             LV_CUDA(s, lvk_bounds_scatter(s->dev, s->bufs, s->force_kernel == LV_FORCE_PACKED, s->stream));
         }
@@ -230,6 +264,13 @@ int enqueue_rebuild_and_forces(lv_sim *s)
 
 int enqueue_step(lv_sim *s)
 {
+    if (s->list_cap > 0) {
+        for (int k = 0; k < LV_N_STAGES; ++k) {
+            int rc = enqueue_stage(s, k, true);
+            if (rc != LV_OK) return rc;
+        }
+        return LV_OK;
+    }
     int rc = enqueue_rebuild_and_forces(s);
     if (rc != LV_OK) return rc;
     return enqueue_stage(s, 4);
@@ -240,7 +281,7 @@ int enqueue_step_timed(lv_sim *s, cudaEvent_t *ev)
 {
     LV_CUDA(s, cudaEventRecord(ev[0], s->stream));
     for (int k = 0; k < LV_N_STAGES; ++k) {
-        int rc = enqueue_stage(s, k);
+        int rc = enqueue_stage(s, k, s->list_cap > 0);
         if (rc != LV_OK) return rc;
         LV_CUDA(s, cudaEventRecord(ev[k + 1], s->stream));
     }
@@ -264,7 +305,7 @@ int build_graph(lv_sim *s)
 {
     if (s->stream == nullptr || s->n == 0) return LV_OK;   // legacy stream: direct launches
     LV_CUDA(s, cudaStreamBeginCapture(s->stream, cudaStreamCaptureModeRelaxed));
-    s->hashed = s->sort_mode == LV_SORT_COUNTING;    // the graph is the steady-state step
+    s->hashed = s->sort_mode == LV_SORT_COUNTING && s->list_cap == 0;   // the graph is the steady-state step
     int rc = enqueue_step(s);
     s->hashed = false;
     cudaGraph_t g = nullptr;
@@ -409,6 +450,27 @@ int lv_set_option(lv_sim *s, int option, int value)
     }
 }
 
+int lv_set_neighbour_list(lv_sim *s, double skin, int capacity)
+{
+    if (!s || !(skin >= 0.0) || capacity < 0 || capacity > (1 << 16)) return LV_E_ARG;
+    if (s->bound) return LV_E_ORDER;
+    if (capacity > 0 && !(skin > 0.0)) return LV_E_ARG;
+    s->skin = capacity > 0 ? skin : 0.0;
+    s->list_cap = capacity;
+    return LV_OK;
+}
+
+int lv_get_rebuild_count(lv_sim *s, int64_t *rebuilds)
+{
+    if (!s || !rebuilds) return LV_E_ARG;
+    if (!s->bound) return LV_E_ORDER;
+    LvDevState h;
+    LV_CUDA(s, cudaMemcpyAsync(&h, s->bufs.st, sizeof(h), cudaMemcpyDeviceToHost, s->stream));
+    LV_CUDA(s, cudaStreamSynchronize(s->stream));
+    *rebuilds = (int64_t)h.n_rebuilds;
+    return LV_OK;
+}
+
 size_t lv_workspace_bytes(const lv_sim *cs)
 {
     lv_sim *s = const_cast<lv_sim *>(cs);
@@ -422,6 +484,7 @@ int lv_bind(lv_sim *s, void *workspace_dev, size_t workspace_bytes, void *cuda_s
     if (!s) return LV_E_ARG;
     if (!s->types_set || !s->sched_set) return LV_E_ORDER;
     if (s->bound) return LV_E_ORDER;
+    if (s->list_cap > 0 && s->sort_mode != LV_SORT_COUNTING) return LV_E_ARG;
     int rc = derive_grid(s);
     if (rc != LV_OK) return rc;
     const Layout L = layout_of(s);
@@ -443,6 +506,9 @@ int lv_bind(lv_sim *s, void *workspace_dev, size_t workspace_bytes, void *cuda_s
     B.scan_tile = (unsigned long long *)(w + L.scan_tile);
     B.scan_ticket = (unsigned int *)(w + L.scan_ticket);
     B.posP = (float *)(w + L.posP);
+    B.list = (uint32_t *)(w + L.list);
+    B.list_rows = (uint32_t *)(w + L.list_rows);
+    B.pos_ref = (float4 *)(w + L.pos_ref);
     s->ws_bytes = L.total;
     s->stream = (cudaStream_t)cuda_stream;
     derive_tables(s);
@@ -489,6 +555,8 @@ int lv_step(lv_sim *s, int n)
     if (!s || n < 0) return LV_E_ARG;
     if (!s->bound || !s->state_set) return LV_E_ORDER;
     if (s->n == 0) return LV_OK;
+    // after the update kernel A has the slot order of `force`; in list mode B may be stale
+    if (n > 0) s->force_order_b = false;
     if (s->tim_cap > 0) {
         if (n > s->tim_cap - s->tim_used) return LV_E_ARG;
         for (int k = 0; k < n; ++k) {
@@ -500,8 +568,8 @@ int lv_step(lv_sim *s, int n)
     }
     for (int k = 0; k < n; ++k) {
         if (s->graph_exec) {
-            if (s->sort_mode == LV_SORT_COUNTING && !s->hashed) {
-                LV_CUDA(s, lvk_hash_count(s->dev, s->bufs, s->stream));
+            if (s->sort_mode == LV_SORT_COUNTING && s->list_cap == 0 && !s->hashed) {
+                LV_CUDA(s, lvk_hash_count(s->dev, s->bufs, false, s->stream));
                 s->hashed = true;        // and the graph's update kernel leaves it true
             }
             LV_CUDA(s, cudaGraphLaunch(s->graph_exec, s->stream));
@@ -518,6 +586,7 @@ int lv_compute_forces(lv_sim *s)
     if (!s) return LV_E_ARG;
     if (!s->bound || !s->state_set) return LV_E_ORDER;
     if (s->n == 0) return LV_OK;
+    s->force_order_b = true;
     return enqueue_rebuild_and_forces(s);
 }
 
@@ -557,7 +626,8 @@ int lv_get_state(lv_sim *s, float *pos_xyz, float *vel_xyz, int32_t *type, doubl
     LV_CUDA(s, cudaStreamSynchronize(s->stream));
     if (step) *step = (int64_t)h.step;
     if (R) *R = lv_radius_of(s->sched_mode, s->R0, s->R1, s->sched_steps, h.step);
-    return (h.status & LV_ST_NONFINITE) ? LV_E_NONFINITE : LV_OK;
+    if (h.status & LV_ST_NONFINITE) return LV_E_NONFINITE;
+    return (h.status & LV_ST_LIST_OVERFLOW) ? LV_E_CAPACITY : LV_OK;
 }
 
 int lv_get_forces(lv_sim *s, float *force_xyz, int32_t *neigh_count, int on_device)
@@ -567,12 +637,12 @@ int lv_get_forces(lv_sim *s, float *force_xyz, int32_t *neigh_count, int on_devi
     const size_t n = (size_t)s->n;
     if (n > 0 && (force_xyz || neigh_count)) {
         if (on_device) {
-            LV_CUDA(s, lvk_unpack_forces(s->dev, s->bufs, force_xyz, neigh_count, s->stream));
+            LV_CUDA(s, lvk_unpack_forces(s->dev, s->bufs, s->force_order_b, force_xyz, neigh_count, s->stream));
         } else {
             unsigned char *stg = s->bufs.staging;
             float *df = (float *)stg;
             int32_t *dc = (int32_t *)(stg + 12 * n);
-            LV_CUDA(s, lvk_unpack_forces(s->dev, s->bufs, force_xyz ? df : nullptr,
+            LV_CUDA(s, lvk_unpack_forces(s->dev, s->bufs, s->force_order_b, force_xyz ? df : nullptr,
                                          neigh_count ? dc : nullptr, s->stream));
             if (force_xyz) LV_CUDA(s, cudaMemcpyAsync(force_xyz, df, 12 * n, cudaMemcpyDeviceToHost, s->stream));
             if (neigh_count) LV_CUDA(s, cudaMemcpyAsync(neigh_count, dc, 4 * n, cudaMemcpyDeviceToHost, s->stream));
@@ -639,7 +709,7 @@ int lv_step_profiled(lv_sim *s, float *ms_out)
     cudaError_t e = cudaSuccess;
     e = cudaEventRecord(ev[0], s->stream);
     for (int k = 0; k < LV_N_STAGES && e == cudaSuccess && rc == LV_OK; ++k) {
-        rc = enqueue_stage(s, k);
+        rc = enqueue_stage(s, k, s->list_cap > 0);
         if (rc == LV_OK) e = cudaEventRecord(ev[k + 1], s->stream);
     }
     if (e == cudaSuccess) e = cudaStreamSynchronize(s->stream);
@@ -740,6 +810,7 @@ const char *lv_strerror(int code)
     case LV_E_ARG: return "bad argument";
     case LV_E_ORDER: return "call order violated";
     case LV_E_WORKSPACE: return "workspace too small or misaligned";
+    case LV_E_CAPACITY: return "skin neighbour list overflowed: raise the capacity";
     case LV_E_CUDA: return "CUDA runtime error";
     case LV_E_NONFINITE: return "non-finite position or velocity";
     case LV_E_NOMEM: return "host allocation failed";

@@ -38,6 +38,7 @@ struct LvDev {
     LvTypeDev type[LV_MAX_TYPES];
     LvGridDev grid[LV_MAX_TYPES];
     int8_t w[LV_MAX_TYPES * LV_MAX_TYPES];
+    int8_t wl[LV_MAX_TYPES * LV_MAX_TYPES];   // stencil half-widths for r_c,ab + skin (list build)
     float dt, g;
     float om2[3];
     int32_t sched_mode;
@@ -47,6 +48,10 @@ struct LvDev {
     double radius_d[LV_MAX_TYPES];
     uint32_t seed_lo, seed_hi;
     uint32_t n_scan_tiles;   // tiles of the cell-count scan (counting sort)
+    // skin neighbour list (lv_set_neighbour_list); list_cap = 0: off
+    int32_t list_cap;        // entries per NP
+    float skin;              // list radius = r_c,ab + skin
+    float half_skin2;        // rebuild when an NP has moved farther than this (squared) since the build
 };
 
 // Device-resident scalars.
@@ -54,6 +59,12 @@ struct LvDevState {
     long long step;        // index of the next step to take
     unsigned int status;   // LV_ST_* bits, sticky
     unsigned int ticket;   // blocks of k_update that have read `step`
+    // skin list: rebuild[n & 1] != 0 -> step n rebuilds the cell structures and the list.
+    // The update of step n raises rebuild[(n + 1) & 1] and, once every block has read
+    // rebuild[n & 1], clears it for step n + 2.
+    unsigned int rebuild[2];
+    unsigned int n_rebuilds;   // rebuilds since lv_set_state
+    unsigned int pad;
 };
 
 struct LvBufs {
@@ -76,6 +87,12 @@ struct LvBufs {
     // 32 bytes {x0, x1, y0, y1, z0, z1, w0, w1}; slots n .. 2*ceil(n/2)+1 are dummies far
     // outside every cut-off.  Written by the gather only when that kernel is selected.
     float *posP;
+    // skin neighbour list: warp w of 32 consecutive slots owns list[(w * cap + t) * 32 + lane],
+    // t < list_rows[w] (entries past an NP's own count hold its own slot); pos_ref = positions
+    // at the last build.
+    uint32_t *list;
+    uint32_t *list_rows;
+    float4 *pos_ref;
 };
 
 // droplet radius after n steps (step (iii)); fp64 on host and device
@@ -95,10 +112,15 @@ constexpr int kScanTile = 4096;   // cells per tile of the cell-count scan
 cudaError_t lvk_hash(const LvDev &P, const LvBufs &B, cudaStream_t st);
 cudaError_t lvk_bounds_scatter(const LvDev &P, const LvBufs &B, bool packed, cudaStream_t st);
 // counting sort (one radix digit = the whole key): hash + count, scan, place, rank + gather
-cudaError_t lvk_hash_count(const LvDev &P, const LvBufs &B, cudaStream_t st);
-cudaError_t lvk_scan_cells(const LvDev &P, const LvBufs &B, cudaStream_t st);
-cudaError_t lvk_place(const LvDev &P, const LvBufs &B, cudaStream_t st);
-cudaError_t lvk_rank_gather(const LvDev &P, const LvBufs &B, bool packed, cudaStream_t st);
+// guarded = true (skin-list steps): the kernel returns at once unless this step rebuilds
+cudaError_t lvk_hash_count(const LvDev &P, const LvBufs &B, bool guarded, cudaStream_t st);
+cudaError_t lvk_scan_cells(const LvDev &P, const LvBufs &B, bool guarded, cudaStream_t st);
+cudaError_t lvk_place(const LvDev &P, const LvBufs &B, bool guarded, cudaStream_t st);
+cudaError_t lvk_rank_gather(const LvDev &P, const LvBufs &B, bool packed, bool guarded, cudaStream_t st);
+// skin list: build from the cell structures (guarded), force from the list, update in list order
+cudaError_t lvk_list_build(const LvDev &P, const LvBufs &B, cudaStream_t st);
+cudaError_t lvk_pair_force_list(const LvDev &P, const LvBufs &B, cudaStream_t st);
+cudaError_t lvk_update_list(const LvDev &P, const LvBufs &B, cudaStream_t st);
 cudaError_t lvk_keys_sorted(const LvDev &P, const LvBufs &B, uint32_t *out, cudaStream_t st);
 cudaError_t lvk_pair_force(const LvDev &P, const LvBufs &B, int variant, cudaStream_t st);
 // hash_next: also hash + histogram the new positions for the next step's counting sort
@@ -107,8 +129,9 @@ cudaError_t lvk_pack_state(const LvDev &P, const LvBufs &B, const float *pos, co
                            const int32_t *type, long long step, cudaStream_t st);
 cudaError_t lvk_unpack_state(const LvDev &P, const LvBufs &B, float *pos, float *vel,
                              int32_t *type, cudaStream_t st);
-cudaError_t lvk_unpack_forces(const LvDev &P, const LvBufs &B, float *force, int32_t *count,
-                              cudaStream_t st);
+// order_b: `force` is in the slot order of B (ids in velB), else of A (ids in velA)
+cudaError_t lvk_unpack_forces(const LvDev &P, const LvBufs &B, bool order_b, float *force,
+                              int32_t *count, cudaStream_t st);
 cudaError_t lvk_ids_sorted(const LvDev &P, const LvBufs &B, uint32_t *ids, cudaStream_t st);
 
 // ---- sort (lv_sort.cu): stable LSD radix sort of (key, val) over end_bit bits

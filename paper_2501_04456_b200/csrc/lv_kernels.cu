@@ -14,6 +14,13 @@ namespace {
 
 constexpr int kThreads = 128;
 
+// Skin-list steps run the cell rebuild only when the device-side flag of this step is
+// raised (LvDevState::rebuild); `guard` is null on every other path.
+__device__ __forceinline__ bool skipped(const LvDevState *guard)
+{
+    return guard != nullptr && guard->rebuild[guard->step & 1] == 0u;
+}
+
 __device__ __forceinline__ int cell_coord(float x, float lo, float inv_h, int G)
 {
     // fp32 contract #1: t = fl(fl(x - lo) * inv_h), clamp(floor t), NaN -> 0
@@ -119,8 +126,9 @@ __global__ void __launch_bounds__(kThreads)
 k_hash_count(const __grid_constant__ LvDev P, const float4 *__restrict__ pos,
              uint32_t *__restrict__ key, uint32_t *__restrict__ rank, uint32_t *__restrict__ cnt,
              unsigned long long *__restrict__ scan_tile, unsigned int *__restrict__ scan_ticket,
-             LvDevState *st)
+             LvDevState *st, const LvDevState *guard)
 {
+    if (skipped(guard)) return;
     int i = blockIdx.x * kThreads + threadIdx.x;
     if (i < (int)P.n_scan_tiles) scan_tile[i] = 0ull;   // re-arm the scan that follows
     if (i == 0) *scan_ticket = 0u;
@@ -148,8 +156,10 @@ constexpr int kScanItems = kScanTile / kScanThreads;   // 16
 
 __global__ void __launch_bounds__(kScanThreads)
 k_scan_cells(uint32_t n_items, uint32_t *__restrict__ cnt, uint32_t *__restrict__ off,
-             volatile unsigned long long *scan_tile, unsigned int *scan_ticket)
+             volatile unsigned long long *scan_tile, unsigned int *scan_ticket,
+             const LvDevState *guard)
 {
+    if (skipped(guard)) return;
     __shared__ uint32_t s_warp[kScanThreads / 32];
     __shared__ uint32_t s_tile, s_excl;
     if (threadIdx.x == 0) s_tile = atomicAdd(scan_ticket, 1u);   // tiles start in ticket order
@@ -237,8 +247,9 @@ k_scan_cells(uint32_t n_items, uint32_t *__restrict__ cnt, uint32_t *__restrict_
 
 __global__ void __launch_bounds__(kThreads)
 k_place(int n, const uint32_t *__restrict__ key, const uint32_t *__restrict__ rank,
-        const uint32_t *__restrict__ off, uint32_t *__restrict__ arrival)
+        const uint32_t *__restrict__ off, uint32_t *__restrict__ arrival, const LvDevState *guard)
 {
+    if (skipped(guard)) return;
     int i = blockIdx.x * kThreads + threadIdx.x;
     if (i < n) arrival[off[key[i]] + rank[i]] = (uint32_t)i;
 }
@@ -247,8 +258,10 @@ __global__ void __launch_bounds__(kThreads)
 k_rank_gather(int n, const uint32_t *__restrict__ key, const uint32_t *__restrict__ off,
               const uint32_t *__restrict__ arrival, uint32_t *__restrict__ perm,
               const float4 *__restrict__ posA, const float4 *__restrict__ velA,
-              float4 *__restrict__ posB, float4 *__restrict__ velB, float *__restrict__ posP)
+              float4 *__restrict__ posB, float4 *__restrict__ velB, float *__restrict__ posP,
+              float4 *__restrict__ pos_ref, const LvDevState *guard)
 {
+    if (skipped(guard)) return;
     int k = blockIdx.x * kThreads + threadIdx.x;
     if (k >= n) return;
     const uint32_t v = arrival[k];
@@ -262,6 +275,7 @@ k_rank_gather(int n, const uint32_t *__restrict__ key, const uint32_t *__restric
     posB[dst] = p;
     velB[dst] = u;
     if (posP) store_packed(posP, (int)dst, n, p);
+    if (pos_ref) pos_ref[dst] = p;      // skin list: displacements are measured from here
 }
 
 __global__ void __launch_bounds__(kThreads)
@@ -555,23 +569,34 @@ __device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c)
     return r;
 }
 
-template <bool kCharged, bool kPacked>
+// kMode 0: forces, scalar walk.  1: forces, packed walk.  2: no forces -- the same row and
+// walk phases with the cut-off widened by the skin EMIT the in-range slots into the lane's
+// column of its warp's tile of the skin neighbour list (lv_set_neighbour_list).
+template <bool kCharged, int kMode>
 __global__ void __launch_bounds__(kSThreads, LV_S_MINBLOCKS)
 k_pair_force_s(const __grid_constant__ LvDev P, const float4 *__restrict__ pos,
                const uint32_t *__restrict__ off, float4 *__restrict__ force,
-               const float *__restrict__ posP)
+               const float *__restrict__ posP, uint32_t *__restrict__ list,
+               uint32_t *__restrict__ list_rows, LvDevState *st)
 {
+    constexpr bool kPacked = kMode == 1;
+    constexpr bool kList = kMode == 2;
+    if (kList && skipped(st)) return;
     __shared__ LvPair s_pair[LV_MAX_TYPES * LV_MAX_TYPES];
     __shared__ int8_t s_w[LV_MAX_TYPES * LV_MAX_TYPES];
     __shared__ uint2 s_seg[kSegCap * kSThreads];
     for (int t = threadIdx.x; t < LV_MAX_TYPES * LV_MAX_TYPES; t += kSThreads) {
         s_pair[t] = P.pair[t];
-        s_w[t] = P.w[t];
+        s_w[t] = kList ? P.wl[t] : P.w[t];
     }
     __syncthreads();
-    const int i = P.n - 1 - (int)(blockIdx.x * kSThreads + threadIdx.x);
+    const int gtid = (int)(blockIdx.x * kSThreads + threadIdx.x);
+    const int i = P.n - 1 - gtid;
     const bool live = i >= 0;
     const uint32_t self = live ? (uint32_t)i : 0u;
+    // list mode: the lane's column of its warp's tile, and whether it overflowed
+    uint32_t *col = kList ? list + ((size_t)(gtid >> 5) * P.list_cap) * 32u + (gtid & 31) : nullptr;
+    bool overflow = false;
     const float4 pi = pos[self];
     const int a = live ? __float_as_int(pi.w) : 0;
     const LvPair *pair_a = s_pair + a * LV_MAX_TYPES;
@@ -613,6 +638,14 @@ k_pair_force_s(const __grid_constant__ LvDev P, const float4 *__restrict__ pos,
                 const float dz = __fsub_rn(pi.z, pj[u].z);
                 const float r2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
                 const bool in = r2 < rc2 && jj[u] != self;           // fp32 contract #2
+                if (kList) {
+                    if (in) {
+                        if (cnt < P.list_cap) col[(size_t)cnt * 32u] = jj[u];
+                        else overflow = true;
+                        cnt += cnt < P.list_cap ? 1 : 0;
+                    }
+                    continue;
+                }
                 const float rinv = rsqrt_approx(r2);
                 const float ir2 = rinv * rinv;
                 const float ir6 = ir2 * ir2 * ir2;
@@ -737,11 +770,15 @@ k_pair_force_s(const __grid_constant__ LvDev P, const float4 *__restrict__ pos,
         const int xlo = max(cx - w, 0), xhi = min(cx + w, g.G - 1);
         // cell units: rounding of contract #1 moves t by < (G + 8) 2^-23; 4x that as margin
         const float marg = (float)(g.G + 8) * 4.76837158e-7f;
-        const float rct2 = pair_a[b].rc2 * 1.0009765625f * (g.inv_h * g.inv_h);
         {
             const LvPair pr = pair_a[b];
             rc2 = pr.rc2; c12 = pr.c12; c6 = pr.c6; qq = pr.qq;
+            if (kList) {        // list radius r_c,ab + skin, rounded up
+                const float rl = __fadd_ru(__fsqrt_ru(pr.rc2), P.skin);
+                rc2 = __fmul_ru(rl, rl);
+            }
         }
+        const float rct2 = rc2 * 1.0009765625f * (g.inv_h * g.inv_h);
         // squared gap (cell units) between the target and the cells at offset d along one axis;
         // cells c >= 1 have a true lower edge and cells c <= G-2 a true upper edge (the clamp
         // only lengthens the two end cells outwards).  Offsets outside the lane's own stencil
@@ -818,6 +855,93 @@ k_pair_force_s(const __grid_constant__ LvDev P, const float4 *__restrict__ pos,
         unpack2(fy2, lo, hi); fy = lo + hi;
         unpack2(fz2, lo, hi); fz = lo + hi;
     }
+    if (kList) {
+        // rows of the tile = the longest column; shorter columns are filled with the lane's
+        // own slot, which the force kernel rejects by j != i
+        const int rows = __reduce_max_sync(kFull, cnt);
+        for (int t = cnt; t < rows; ++t) col[(size_t)t * 32u] = self;
+        if ((gtid & 31) == 0) list_rows[gtid >> 5] = (uint32_t)rows;
+        if (overflow) atomicOr(&st->status, LV_ST_LIST_OVERFLOW);
+        if (gtid == 0) st->n_rebuilds += 1u;
+        return;
+    }
+    if (live) force[i] = make_float4(fx, fy, fz, __int_as_float(cnt));
+}
+
+// Pair force from the skin neighbour list (lv_set_neighbour_list).  Lane = NP, as in the
+// build; the warp reads row t of its tile with ONE coalesced load (32 slot indices), each
+// lane gathers its candidate's position and evaluates contract #2 and the force -- no cell
+// arithmetic, no runs: the instruction stream is the distance test and the force.  The
+// positions are those of the list's slot order: posB on the step that rebuilt, else posA
+// (k_update keeps that order until the next rebuild).
+constexpr int kLChunk = 4;
+
+template <bool kCharged>
+__global__ void __launch_bounds__(kSThreads)
+k_pair_force_list(const __grid_constant__ LvDev P, const float4 *__restrict__ posA,
+                  const float4 *__restrict__ posB, const uint32_t *__restrict__ list,
+                  const uint32_t *__restrict__ list_rows, float4 *__restrict__ force,
+                  const LvDevState *st)
+{
+    __shared__ LvPair s_pair[LV_MAX_TYPES * LV_MAX_TYPES];
+    for (int t = threadIdx.x; t < LV_MAX_TYPES * LV_MAX_TYPES; t += kSThreads) s_pair[t] = P.pair[t];
+    __syncthreads();
+    const float4 *__restrict__ pos = st->rebuild[st->step & 1] ? posB : posA;
+    const int gtid = (int)(blockIdx.x * kSThreads + threadIdx.x);
+    const int i = P.n - 1 - gtid;
+    const bool live = i >= 0;
+    const uint32_t self = live ? (uint32_t)i : 0u;
+    const float4 pi = pos[self];
+    const LvPair *pair_a = s_pair + (live ? __float_as_int(pi.w) : 0) * LV_MAX_TYPES;
+    const uint32_t *col = list + ((size_t)(gtid >> 5) * P.list_cap) * 32u + (gtid & 31);
+    const int rows = (int)list_rows[gtid >> 5];
+    float fx = 0.f, fy = 0.f, fz = 0.f;
+    int cnt = 0;
+
+    // three chunks in flight: the slot indices of chunk c + 2 and the positions of chunk
+    // c + 1 are loading while chunk c is evaluated (the gather is a dependent load pair)
+    auto fetch_idx = [&](int t, uint32_t (&jj)[kLChunk]) {
+#pragma unroll
+        for (int u = 0; u < kLChunk; ++u) jj[u] = t + u < rows ? __ldg(col + (size_t)(t + u) * 32u) : self;
+    };
+    auto fetch_pos = [&](const uint32_t (&jj)[kLChunk], float4 (&pj)[kLChunk]) {
+#pragma unroll
+        for (int u = 0; u < kLChunk; ++u) pj[u] = __ldg(pos + jj[u]);
+    };
+    auto eval = [&](const uint32_t (&jj)[kLChunk], const float4 (&pj)[kLChunk]) {
+#pragma unroll
+        for (int u = 0; u < kLChunk; ++u) {
+            const LvPair pr = pair_a[__float_as_int(pj[u].w)];
+            const float dx = __fsub_rn(pi.x, pj[u].x);
+            const float dy = __fsub_rn(pi.y, pj[u].y);
+            const float dz = __fsub_rn(pi.z, pj[u].z);
+            const float r2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
+            const bool in = r2 < pr.rc2 && jj[u] != self;            // fp32 contract #2
+            const float rinv = rsqrt_approx(r2);
+            const float ir2 = rinv * rinv;
+            const float ir6 = ir2 * ir2 * ir2;
+            float f = fmaf(pr.c12, ir6, -pr.c6) * ir6;
+            if (kCharged) f = fmaf(pr.qq, rinv, f);
+            f *= ir2;
+            f = in ? f : 0.0f;
+            fx = fmaf(f, dx, fx);
+            fy = fmaf(f, dy, fy);
+            fz = fmaf(f, dz, fz);
+            cnt += in ? 1 : 0;
+        }
+    };
+    uint32_t ja[kLChunk], jb[kLChunk], jc[kLChunk];
+    float4 pa[kLChunk], pb[kLChunk], pc[kLChunk];
+    fetch_idx(0, ja);
+    fetch_idx(kLChunk, jb);
+    fetch_pos(ja, pa);
+    for (int t = 0; t < rows; t += 3 * kLChunk) {
+        fetch_idx(t + 2 * kLChunk, jc); fetch_pos(jb, pb); eval(ja, pa);
+        if (t + kLChunk >= rows) break;
+        fetch_idx(t + 3 * kLChunk, ja); fetch_pos(jc, pc); eval(jb, pb);
+        if (t + 2 * kLChunk >= rows) break;
+        fetch_idx(t + 4 * kLChunk, jb); fetch_pos(ja, pa); eval(jc, pc);
+    }
     if (live) force[i] = make_float4(fx, fy, fz, __int_as_float(cnt));
 }
 
@@ -844,13 +968,18 @@ __device__ __forceinline__ float u01(uint32_t w)
 
 // kHash: also do A2 + the histogram of the NEXT step's counting sort on the new position
 // (k_hash_count's work, same fp32 contract #1), so a steady-state step has no hash kernel.
-template <bool kHash>
+// kList (skin neighbour list): the slot order is that of the last rebuild, so the state is
+// read from B on the step that rebuilt and from A (in place) otherwise; an NP that has moved
+// farther than half the skin from its position at the build raises the rebuild flag of the
+// next step.
+template <bool kHash, bool kList>
 __global__ void __launch_bounds__(kThreads)
-k_update(const __grid_constant__ LvDev P, const float4 *__restrict__ posB,
-         const float4 *__restrict__ velB, const float4 *__restrict__ force,
-         float4 *__restrict__ posA, float4 *__restrict__ velA, LvDevState *st,
+k_update(const __grid_constant__ LvDev P, const float4 *__restrict__ posB_,
+         const float4 *__restrict__ velB_, const float4 *__restrict__ force,
+         float4 *posA, float4 *velA, LvDevState *st,
          uint32_t *__restrict__ key, uint32_t *__restrict__ rank, uint32_t *__restrict__ cnt,
-         unsigned long long *__restrict__ scan_tile, unsigned int *__restrict__ scan_ticket)
+         unsigned long long *__restrict__ scan_tile, unsigned int *__restrict__ scan_ticket,
+         const float4 *__restrict__ pos_ref)
 {
     int i = blockIdx.x * kThreads + threadIdx.x;
     if (kHash) {
@@ -858,13 +987,17 @@ k_update(const __grid_constant__ LvDev P, const float4 *__restrict__ posB,
         if (i == 0) *scan_ticket = 0u;
     }
     const long long n = st->step;                      // index of this step
+    const bool rebuilt = kList ? st->rebuild[n & 1] != 0u : true;
     __syncthreads();
     // the block that takes the last ticket has seen every block read `step`
     if (threadIdx.x == 0 && atomicAdd(&st->ticket, 1u) == gridDim.x - 1) {
         st->ticket = 0u;
         st->step = n + 1;
+        if (kList) st->rebuild[n & 1] = 0u;            // ... and this step's rebuild flag
     }
     if (i >= P.n) return;
+    const float4 *posB = rebuilt ? posB_ : posA;
+    const float4 *velB = rebuilt ? velB_ : velA;
     const double Rd = lv_radius_of(P.sched_mode, P.R0, P.R1, P.sched_steps, n + 1);  // (iii), R9
     const float4 p = posB[i];
     const float4 v = velB[i];
@@ -919,6 +1052,11 @@ k_update(const __grid_constant__ LvDev P, const float4 *__restrict__ posB,
     velA[i] = make_float4(vx, vy, vz, v.w);
     const float chk = (x + y + z) + (vx + vy + vz);
     if (!(fabsf(chk) <= 3.0e38f)) atomicOr(&st->status, LV_ST_NONFINITE);
+    if (kList) {
+        const float4 r = pos_ref[i];
+        const float ex = x - r.x, ey = y - r.y, ez = z - r.z;
+        if (!(fmaf(ez, ez, fmaf(ey, ey, ex * ex)) <= P.half_skin2)) st->rebuild[(n + 1) & 1] = 1u;
+    }
     if (kHash) {
         const LvGridDev g = P.grid[a];
         const int cx = cell_coord(x, g.lo, g.inv_h, g.G);
@@ -940,7 +1078,12 @@ k_pack_state(int n, const float *__restrict__ pos, const float *__restrict__ vel
              float4 *__restrict__ velA, LvDevState *st, long long step)
 {
     int i = blockIdx.x * kThreads + threadIdx.x;
-    if (i == 0) { st->step = step; st->status = 0u; st->ticket = 0u; }
+    if (i == 0) {
+        st->step = step; st->status = 0u; st->ticket = 0u;
+        st->rebuild[step & 1] = 1u;            // skin list: the first step builds it
+        st->rebuild[(step + 1) & 1] = 0u;
+        st->n_rebuilds = 0u;
+    }
     if (i >= n) return;
     posA[i] = make_float4(pos[3 * i], pos[3 * i + 1], pos[3 * i + 2], __int_as_float(type[i]));
     velA[i] = make_float4(vel[3 * i], vel[3 * i + 1], vel[3 * i + 2], __uint_as_float((uint32_t)i));
@@ -996,6 +1139,14 @@ cudaError_t lvk_bounds_scatter(const LvDev &P, const LvBufs &B, bool packed, cud
     return cudaGetLastError();
 }
 
+static bool any_charge(const LvDev &P)
+{
+    bool charged = false;
+    for (int a = 0; a < P.n_types; ++a)
+        for (int b = 0; b < P.n_types; ++b) charged |= P.pair[a * LV_MAX_TYPES + b].qq != 0.0f;
+    return charged;
+}
+
 cudaError_t lvk_pair_force(const LvDev &P, const LvBufs &B, int variant, cudaStream_t st)
 {
     if (variant == 0)
@@ -1004,51 +1155,79 @@ cudaError_t lvk_pair_force(const LvDev &P, const LvBufs &B, int variant, cudaStr
         k_pair_force_q<<<(P.n + kFThreads - 1) / kFThreads, kFThreads, 0, st>>>(P, B.posB, B.cell_off,
                                                                              B.force);
     else {
-        bool charged = false;
-        for (int a = 0; a < P.n_types; ++a)
-            for (int b = 0; b < P.n_types; ++b) charged |= P.pair[a * LV_MAX_TYPES + b].qq != 0.0f;
+        const bool charged = any_charge(P);
         const int blocks = (P.n + kSThreads - 1) / kSThreads;
         if (variant == 3) {
             if (charged)
-                k_pair_force_s<true, true><<<blocks, kSThreads, 0, st>>>(P, B.posB, B.cell_off, B.force, B.posP);
+                k_pair_force_s<true, 1><<<blocks, kSThreads, 0, st>>>(P, B.posB, B.cell_off, B.force,
+                                                                      B.posP, nullptr, nullptr, nullptr);
             else
-                k_pair_force_s<false, true><<<blocks, kSThreads, 0, st>>>(P, B.posB, B.cell_off, B.force, B.posP);
+                k_pair_force_s<false, 1><<<blocks, kSThreads, 0, st>>>(P, B.posB, B.cell_off, B.force,
+                                                                       B.posP, nullptr, nullptr, nullptr);
         } else {
             if (charged)
-                k_pair_force_s<true, false><<<blocks, kSThreads, 0, st>>>(P, B.posB, B.cell_off, B.force, nullptr);
+                k_pair_force_s<true, 0><<<blocks, kSThreads, 0, st>>>(P, B.posB, B.cell_off, B.force,
+                                                                      nullptr, nullptr, nullptr, nullptr);
             else
-                k_pair_force_s<false, false><<<blocks, kSThreads, 0, st>>>(P, B.posB, B.cell_off, B.force, nullptr);
+                k_pair_force_s<false, 0><<<blocks, kSThreads, 0, st>>>(P, B.posB, B.cell_off, B.force,
+                                                                       nullptr, nullptr, nullptr, nullptr);
         }
     }
     return cudaGetLastError();
 }
 
-cudaError_t lvk_hash_count(const LvDev &P, const LvBufs &B, cudaStream_t st)
+// skin list: tiles are indexed by the launch's warp id, so build and force use the same grid
+cudaError_t lvk_list_build(const LvDev &P, const LvBufs &B, cudaStream_t st)
+{
+    const int blocks = (P.n + kSThreads - 1) / kSThreads;
+    k_pair_force_s<false, 2><<<blocks, kSThreads, 0, st>>>(P, B.posB, B.cell_off, nullptr, nullptr,
+                                                           B.list, B.list_rows, B.st);
+    return cudaGetLastError();
+}
+
+cudaError_t lvk_pair_force_list(const LvDev &P, const LvBufs &B, cudaStream_t st)
+{
+    const int blocks = (P.n + kSThreads - 1) / kSThreads;
+    if (any_charge(P))
+        k_pair_force_list<true><<<blocks, kSThreads, 0, st>>>(P, B.posA, B.posB, B.list, B.list_rows,
+                                                              B.force, B.st);
+    else
+        k_pair_force_list<false><<<blocks, kSThreads, 0, st>>>(P, B.posA, B.posB, B.list, B.list_rows,
+                                                               B.force, B.st);
+    return cudaGetLastError();
+}
+
+cudaError_t lvk_hash_count(const LvDev &P, const LvBufs &B, bool guarded, cudaStream_t st)
 {
     const int m = P.n > (int)P.n_scan_tiles ? P.n : (int)P.n_scan_tiles;
     k_hash_count<<<blocks_for(m), kThreads, 0, st>>>(P, B.posA, B.key_in, B.val_in, B.cell_cnt,
-                                                     B.scan_tile, B.scan_ticket, B.st);
+                                                     B.scan_tile, B.scan_ticket, B.st,
+                                                     guarded ? B.st : nullptr);
     return cudaGetLastError();
 }
 
-cudaError_t lvk_scan_cells(const LvDev &P, const LvBufs &B, cudaStream_t st)
+cudaError_t lvk_scan_cells(const LvDev &P, const LvBufs &B, bool guarded, cudaStream_t st)
 {
     k_scan_cells<<<P.n_scan_tiles, kScanThreads, 0, st>>>(P.n_cells + 1u, B.cell_cnt, B.cell_off,
-                                                          B.scan_tile, B.scan_ticket);
+                                                          B.scan_tile, B.scan_ticket,
+                                                          guarded ? B.st : nullptr);
     return cudaGetLastError();
 }
 
-cudaError_t lvk_place(const LvDev &P, const LvBufs &B, cudaStream_t st)
+cudaError_t lvk_place(const LvDev &P, const LvBufs &B, bool guarded, cudaStream_t st)
 {
-    k_place<<<blocks_for(P.n), kThreads, 0, st>>>(P.n, B.key_in, B.val_in, B.cell_off, B.key_out);
+    k_place<<<blocks_for(P.n), kThreads, 0, st>>>(P.n, B.key_in, B.val_in, B.cell_off, B.key_out,
+                                                  guarded ? B.st : nullptr);
     return cudaGetLastError();
 }
 
-cudaError_t lvk_rank_gather(const LvDev &P, const LvBufs &B, bool packed, cudaStream_t st)
+cudaError_t lvk_rank_gather(const LvDev &P, const LvBufs &B, bool packed, bool guarded, cudaStream_t st)
 {
     k_rank_gather<<<blocks_for(P.n), kThreads, 0, st>>>(P.n, B.key_in, B.cell_off, B.key_out, B.val_out,
                                                         B.posA, B.velA, B.posB, B.velB,
-                                                        packed ? B.posP : nullptr);
+                                                        packed ? B.posP : nullptr,
+                                                        guarded ? B.pos_ref : nullptr,
+                                                        guarded ? B.st : nullptr);
     return cudaGetLastError();
 }
 
@@ -1062,14 +1241,22 @@ cudaError_t lvk_update(const LvDev &P, const LvBufs &B, bool hash_next, cudaStre
 {
     if (hash_next) {
         const int m = P.n > (int)P.n_scan_tiles ? P.n : (int)P.n_scan_tiles;
-        k_update<true><<<blocks_for(m), kThreads, 0, st>>>(P, B.posB, B.velB, B.force, B.posA, B.velA,
-                                                           B.st, B.key_in, B.val_in, B.cell_cnt,
-                                                           B.scan_tile, B.scan_ticket);
+        k_update<true, false><<<blocks_for(m), kThreads, 0, st>>>(
+            P, B.posB, B.velB, B.force, B.posA, B.velA, B.st, B.key_in, B.val_in, B.cell_cnt,
+            B.scan_tile, B.scan_ticket, nullptr);
     } else {
-        k_update<false><<<blocks_for(P.n), kThreads, 0, st>>>(P, B.posB, B.velB, B.force, B.posA,
-                                                            B.velA, B.st, nullptr, nullptr, nullptr,
-                                                            nullptr, nullptr);
+        k_update<false, false><<<blocks_for(P.n), kThreads, 0, st>>>(
+            P, B.posB, B.velB, B.force, B.posA, B.velA, B.st, nullptr, nullptr, nullptr, nullptr,
+            nullptr, nullptr);
     }
+    return cudaGetLastError();
+}
+
+cudaError_t lvk_update_list(const LvDev &P, const LvBufs &B, cudaStream_t st)
+{
+    k_update<false, true><<<blocks_for(P.n), kThreads, 0, st>>>(
+        P, B.posB, B.velB, B.force, B.posA, B.velA, B.st, nullptr, nullptr, nullptr, nullptr, nullptr,
+        B.pos_ref);
     return cudaGetLastError();
 }
 
@@ -1087,10 +1274,11 @@ cudaError_t lvk_unpack_state(const LvDev &P, const LvBufs &B, float *pos, float 
     return cudaGetLastError();
 }
 
-cudaError_t lvk_unpack_forces(const LvDev &P, const LvBufs &B, float *force, int32_t *count,
-                              cudaStream_t st)
+cudaError_t lvk_unpack_forces(const LvDev &P, const LvBufs &B, bool order_b, float *force,
+                              int32_t *count, cudaStream_t st)
 {
-    k_unpack_forces<<<blocks_for(P.n), kThreads, 0, st>>>(P.n, B.force, B.velB, force, count);
+    k_unpack_forces<<<blocks_for(P.n), kThreads, 0, st>>>(P.n, B.force, order_b ? B.velB : B.velA,
+                                                          force, count);
     return cudaGetLastError();
 }
 

@@ -59,6 +59,9 @@ class Workload:
     # cells per cut-off per type (lv_set_grid) measured fastest on B200 for this config
     # (DESIGN.md sec. 7.2); bench.py's default.  A tuning choice, not part of the model.
     tuned_cells_per_cut: Optional[List[int]] = None
+    # (skin, entries per NP) for lv_set_neighbour_list at the START of the schedule, used by
+    # bench.py's skin-list variant; a shrinking droplet needs more capacity later on
+    tuned_neighbour_list: Optional[Sequence[float]] = None
     pos: np.ndarray = field(default=None, repr=False)    # [n,3] float32
     vel: np.ndarray = field(default=None, repr=False)    # [n,3] float32
     type: np.ndarray = field(default=None, repr=False)   # [n] int32
@@ -80,14 +83,16 @@ def _spec(name: str) -> Workload:
                         kT=1.0, dt=0.005, cut_factor=2.5, coulomb_k=0.0, g=0.0,
                         omega2=(0.0, 0.0, 0.0), wall_mode=WALL_ONESIDED,
                         sched_mode=SCHED_CONST, R0=20.0, R1=20.0, sched_steps=0,
-                        seed=1, steps=1000, init="ball", tuned_cells_per_cut=[1])
+                        seed=1, steps=1000, init="ball", tuned_cells_per_cut=[1],
+                        tuned_neighbour_list=(0.3, 64))
     if name == "C2":
         s = [1.0, 1.5]
         return Workload("C2", 32768, s, [1.0, 2.0], [1.0, -1.0], _mass(s), [100.0] * 2,
                         [1.0] * 2, [0.7, 0.3], kT=1.0, dt=0.002, cut_factor=5.0,
                         coulomb_k=0.7, g=0.0, omega2=(0.0, 0.0, 0.0),
                         wall_mode=WALL_ONESIDED, sched_mode=SCHED_LINEAR, R0=60.0, R1=25.0,
-                        sched_steps=10000, seed=2, steps=10000, init="ball", tuned_cells_per_cut=[2, 2])
+                        sched_steps=10000, seed=2, steps=10000, init="ball", tuned_cells_per_cut=[2, 2],
+                        tuned_neighbour_list=(0.4, 256))
     if name == "C3":
         s = [1.0, 1.5, 2.5]
         w2 = 0.005 ** 2
@@ -95,7 +100,8 @@ def _spec(name: str) -> Workload:
                         [100.0] * 3, [2.0] * 3, [0.5, 0.3, 0.2], kT=1.0, dt=0.002,
                         cut_factor=5.0, coulomb_k=0.7, g=0.01, omega2=(w2, w2, 0.0),
                         wall_mode=WALL_ONESIDED, sched_mode=SCHED_LINEAR, R0=150.0, R1=50.0,
-                        sched_steps=20000, seed=3, steps=20000, init="ball", tuned_cells_per_cut=[1, 2, 2])
+                        sched_steps=20000, seed=3, steps=20000, init="ball", tuned_cells_per_cut=[1, 2, 2],
+                        tuned_neighbour_list=(0.5, 256))
     if name == "C4":
         s = [1.0]
         n = 250000
@@ -104,14 +110,16 @@ def _spec(name: str) -> Workload:
                         kT=0.5, dt=0.001, cut_factor=2.5, coulomb_k=0.0, g=0.0,
                         omega2=(0.0, 0.0, 0.0), wall_mode=WALL_ONESIDED,
                         sched_mode=SCHED_CONST, R0=R, R1=R, sched_steps=0,
-                        seed=4, steps=5000, init="fcc", tuned_cells_per_cut=[3])
+                        seed=4, steps=5000, init="fcc", tuned_cells_per_cut=[3],
+                        tuned_neighbour_list=(0.2, 160))
     if name == "C5":
         s = [1.0, 1.2]
         return Workload("C5", 1048576, s, [1.0, 1.0], [0.5, -0.5], _mass(s), [100.0] * 2,
                         [1.0] * 2, [0.5, 0.5], kT=1.0, dt=0.002, cut_factor=4.0,
                         coulomb_k=0.7, g=0.0, omega2=(0.0, 0.0, 0.0),
                         wall_mode=WALL_ONESIDED, sched_mode=SCHED_LINEAR, R0=250.0, R1=120.0,
-                        sched_steps=10000, seed=5, steps=10000, init="ball", tuned_cells_per_cut=[1, 1])
+                        sched_steps=10000, seed=5, steps=10000, init="ball", tuned_cells_per_cut=[1, 1],
+                        tuned_neighbour_list=(0.4, 128))
     raise KeyError(name)
 
 

@@ -1,0 +1,143 @@
+"""Skin neighbour list (lv_set_neighbour_list): same results as the
+per-step cell rebuild -- neighbour counts bit-exact (fp32 contract #2), forces to rounding,
+trajectories within the oracle tolerances -- with rebuilds decided on the device."""
+import numpy as np
+import pytest
+
+from paper_2501_04456_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+FORCE_TOL = 1e-5
+
+
+@pytest.fixture(scope="module")
+def orc():
+    import oracle
+    return oracle
+
+
+@pytest.fixture(scope="module")
+def B():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_2501_04456_b200 import binding
+    binding.load()
+    return binding
+
+
+def force_error(Fg, Fo, So):
+    err = np.abs(Fg.astype(np.float64) - Fo).max(axis=1)
+    nz = So > 0
+    return (err[nz] / So[nz]).max() if nz.any() else 0.0
+
+
+CASES = [  # (config, n, cells_per_cut, skin, capacity)
+    ("C1", None, None, 0.3, 64),
+    ("C3", 20000, [1, 2, 2], 0.5, 256),
+    ("C4", 19999, [2], 0.2, 160),
+    ("C2", 8191, [2, 2], 0.4, 256),
+]
+
+
+@pytest.mark.parametrize("name,n,cpc,skin,cap", CASES)
+def test_first_step_forces_and_counts_against_oracle(B, orc, name, n, cpc, skin, cap):
+    w = W.make_workload(name, n)
+    p = orc.params_from_workload(w)
+    Fo, So, co, _ = orc.pair_forces(p, w.pos, w.type, "cells")
+    sim = B.Simulation.from_workload(w, cells_per_cut=cpc, neighbour_list=(skin, cap))
+    sim.step(1)                                   # builds the list, forces of the initial state
+    Fg, cg = sim.get_forces()
+    assert np.array_equal(cg, co)                 # neighbour counts bit-exact
+    assert force_error(Fg, Fo, So) <= FORCE_TOL
+    assert sim.rebuild_count() == 1
+    sim.get_state()
+    sim.close()
+
+
+@pytest.mark.parametrize("name,n,cpc,skin,cap", CASES)
+def test_list_stays_complete_between_rebuilds(B, name, n, cpc, skin, cap):
+    """At arbitrary later steps the list run's forces and counts equal a fresh cell rebuild of
+    the same state: no in-range pair is ever missing from a list that was built steps ago."""
+    w = W.make_workload(name, n)
+    lst = B.Simulation.from_workload(w, cells_per_cut=cpc, neighbour_list=(skin, cap))
+    cel = B.Simulation.from_workload(w, cells_per_cut=cpc)
+    done = 0
+    for k in (3, 37, 150, 400):
+        lst.step(k - done)
+        done = k
+        x, v, t, R, st = lst.get_state()
+        assert st == k
+        cel.set_state(x, v, t, step=k)
+        cel.compute_forces()
+        Fc, cc = cel.get_forces()
+        lst.step(1)                               # forces of the state at step k
+        done += 1
+        Fl, cl = lst.get_forces()
+        assert np.array_equal(cl, cc), k
+        S = np.abs(Fc).sum(axis=1) + 1e-30
+        # same pairs, different summation order: rounding only (relative to the net force
+        # plus a floor for cancelling terms)
+        assert np.max(np.abs(Fl - Fc).max(axis=1) / (S + np.abs(Fc).max())) <= 1e-4, k
+    r = lst.rebuild_count()
+    assert 1 < r < done, r                        # rebuilt, but not every step
+    assert lst.status() == 0
+    lst.close(); cel.close()
+
+
+def test_hundred_steps_against_oracle(B, orc):
+    w = W.make_workload("C3", 20000)
+    p = orc.params_from_workload(w)
+    xo, vo, bad = orc.step(p, w.pos, w.vel, w.type, step0=0, nsteps=100)
+    assert bad == 0
+    sim = B.Simulation.from_workload(w, cells_per_cut=[1, 2, 2], neighbour_list=(0.5, 256))
+    sim.step(100)
+    x, v, t, R, st = sim.get_state()
+    assert st == 100
+    assert np.linalg.norm(x.astype(np.float64) - xo, axis=1).max() <= 1e-3 * R
+    assert 1 <= sim.rebuild_count() < 100
+    sim.close()
+
+
+def test_split_invariance_and_restart(B):
+    w = W.make_workload("C2", 8191)
+    a = B.Simulation.from_workload(w, cells_per_cut=[2, 2], neighbour_list=(0.4, 256))
+    b = B.Simulation.from_workload(w, cells_per_cut=[2, 2], neighbour_list=(0.4, 256))
+    a.step(60)
+    b.step(23); b.step(1); b.step(36)
+    xa, va, _, _, _ = a.get_state()
+    xb, vb, _, _, _ = b.get_state()
+    assert np.array_equal(xa, xb) and np.array_equal(va, vb)
+    assert a.rebuild_count() == b.rebuild_count()
+    # lv_compute_forces between steps (always the cells) does not disturb the list run
+    b.compute_forces()
+    a.step(40); b.step(40)
+    xa, va, _, _, _ = a.get_state()
+    xb, vb, _, _, _ = b.get_state()
+    assert np.array_equal(xa, xb) and np.array_equal(va, vb)
+    # lv_set_state starts a fresh list
+    a.set_state(w.pos, w.vel, w.type, 0)
+    a.step(60)
+    xc, vc, _, _, _ = a.get_state()
+    b.set_state(w.pos, w.vel, w.type, 0)
+    b.step(60)
+    xd, vd, _, _, _ = b.get_state()
+    assert np.array_equal(xc, xd) and np.array_equal(vc, vd)
+    a.close(); b.close()
+
+
+def test_overflow_is_reported(B):
+    w = W.make_workload("C4", 19999)              # ~50 neighbours per NP
+    sim = B.Simulation.from_workload(w, cells_per_cut=[2], neighbour_list=(0.2, 8))
+    sim.step(1)
+    assert sim.status() & B.ST_LIST_OVERFLOW
+    with pytest.raises(B.LvError) as e:
+        sim.get_state()
+    assert e.value.code == B.E_CAPACITY
+    sim.close()
+
+
+def test_needs_the_counting_sort(B):
+    w = W.make_workload("C1")
+    with pytest.raises(B.LvError):
+        B.Simulation.from_workload(w, options={B.OPT_SORT: B.SORT_RADIX}, neighbour_list=(0.3, 64))
