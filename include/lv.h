@@ -216,6 +216,28 @@ int lv_get_state(lv_sim *s, float *pos_xyz, float *vel_xyz, int32_t *type, doubl
  * device per on_device; either may be NULL.  Synchronises. */
 int lv_get_forces(lv_sim *s, float *force_xyz, int32_t *neigh_count, int on_device);
 
+/* ---- observables of the paper on the device ----------------
+ * Shell index of a distance (fp32 contract #4): (int) fl32(sqrt(r2) * fl32(1/dr))
+ * with r2 as in the in-range predicate; counted iff < n_bins (1..8192, and
+ * 8 n_bins + 64 <= 28 n).  All outputs are host memory, written; any may be NULL.
+ * Both calls synchronise the stream and leave the state unchanged.
+ *
+ * lv_observe_rdf: radial distribution function, Eq. 6.  hist[k] =
+ * ordered pairs (i, j != i) whose distance falls in shell k (each NP in turn is the
+ * "trial particle"); g[k] = (hist[k]/N) / ((N-1) dV_k / V), dV_k the shell volume and V
+ * the droplet volume at the current step; no boundary correction, as printed
+ * (PAPER.md:139).  Rebuilds the cell structures of the current state and walks them. */
+int lv_observe_rdf(lv_sim *s, double dr, int n_bins, uint64_t *hist, double *g);
+
+/* lv_observe_radial: hist[k] = NPs whose distance from the droplet centre falls in shell
+ * k and conc[k] = (hist[k]/N) / (dV_k / V), the normalised concentration of Eq. 8
+ * (PAPER.md:141); centre[3] = Eq. 4, r_g = Eq. 3, d_f = Eq. 2 solved for D_f with
+ * k_f = 1.593 and d_NP the mean NP diameter; n_surf = NPs whose
+ * surface lies within one NP radius of the interface, |x| > R - 2 r_a (the NPs that
+ * enter Eq. 1). */
+int lv_observe_radial(lv_sim *s, double dr, int n_bins, uint64_t *hist, double *conc,
+                      double *centre, double *r_g, double *d_f, int64_t *n_surf);
+
 /* Status bits LV_ST_* (host uint32, written).  Synchronises. */
 int lv_get_status(lv_sim *s, uint32_t *status);
 

@@ -89,6 +89,11 @@ def lib():
         L.lvo_stable_sort_perm.restype = None
         L.lvo_cell_offsets.argtypes = [C.c_int, up, C.c_uint32, up]
         L.lvo_cell_offsets.restype = None
+        L.lvo_rdf_hist.argtypes = [C.c_int, fp, C.c_float, C.c_int, C.POINTER(C.c_uint64)]
+        L.lvo_rdf_hist.restype = None
+        L.lvo_radial_hist.argtypes = [C.c_int, fp, ip, dp, C.c_double, C.c_float, C.c_int,
+                                      C.POINTER(C.c_uint64), dp, C.POINTER(C.c_int64)]
+        L.lvo_radial_hist.restype = None
         L.lvo_sizeof_params.restype = C.c_int
         L.lvo_sizeof_grid.restype = C.c_int
         L.lvo_max_threads.restype = C.c_int
@@ -284,3 +289,37 @@ def cell_structures(g: Grid, x_f32, type_):
     L.lvo_stable_sort_perm(n, _u(key), _u(ks), _u(perm))
     L.lvo_cell_offsets(n, _u(ks), ncell, _u(off))
     return key, ks, perm, off
+
+
+def rdf_hist(x_f32, dr, n_bins):
+    """fp32 contract #4: ordered-pair counts per shell [k dr, (k+1) dr) -> uint64[n_bins]."""
+    x = np.ascontiguousarray(x_f32, dtype=np.float32).reshape(-1, 3)
+    h = np.zeros(int(n_bins), dtype=np.uint64)
+    inv_dr = np.float32(1.0 / float(dr))
+    lib().lvo_rdf_hist(x.shape[0], _f(x), C.c_float(float(inv_dr)), int(n_bins),
+                       h.ctypes.data_as(C.POINTER(C.c_uint64)))
+    return h
+
+
+def radial_hist(x_f32, type_, radius_a, R, dr, n_bins):
+    """-> (NPs per shell around the centre uint64[n_bins], (sum x, sum y, sum z, sum |x|^2),
+    N_surf)."""
+    x = np.ascontiguousarray(x_f32, dtype=np.float32).reshape(-1, 3)
+    t = _ci32(type_)
+    ra = _c64(radius_a)
+    h = np.zeros(int(n_bins), dtype=np.uint64)
+    sums = np.zeros(4)
+    ns = C.c_int64()
+    inv_dr = np.float32(1.0 / float(dr))
+    lib().lvo_radial_hist(x.shape[0], _f(x), _i(t), _d(ra), float(R), C.c_float(float(inv_dr)),
+                          int(n_bins), h.ctypes.data_as(C.POINTER(C.c_uint64)), _d(sums),
+                          C.byref(ns))
+    return h, sums, int(ns.value)
+
+
+def rdf_from_hist(hist, n, R, dr):
+    """Eq. 6 from the ordered-pair counts: g_k = (psi_k / N) / ((N-1) dV_k / V)."""
+    k = np.arange(len(hist), dtype=np.float64)
+    dV = 4.0 / 3.0 * np.pi * (((k + 1) * dr) ** 3 - (k * dr) ** 3)
+    V = 4.0 / 3.0 * np.pi * float(R) ** 3
+    return (np.asarray(hist, dtype=np.float64) / n) / ((n - 1) * dV / V)

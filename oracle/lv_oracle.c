@@ -524,6 +524,54 @@ void lvo_cell_offsets(int n, const uint32_t *key_sorted, uint32_t n_cells, uint3
     }
 }
 
+
+/* ------------------------------------------------------------------ */
+/* Observables as integer histograms.  The bin of a distance
+ * is an integer decided by floating point, so -- as for the cell hash -- it is DEFINED
+ * on the fp32 state by a fixed fp32 expression that both sides evaluate literally
+ * (fp32 contract #4):
+ *     r2 as in contract #2;  r = sqrtf(r2) (correctly rounded);
+ *     bin = (int) fl32(r * inv_dr),  inv_dr = fl32(1 / dr);  counted iff bin < n_bins.
+ * The histograms below are the plain definitions: every ordered pair (Eq. 6: each NP
+ * in turn is the "trial particle"), every NP (Eq. 8).
+ * They are pinned against oracle/observables.py (fp64, np.histogram), itself pinned
+ * against closed forms. */
+void lvo_rdf_hist(int n, const float *x, float inv_dr, int n_bins, uint64_t *hist)
+{
+    for (int b = 0; b < n_bins; ++b) hist[b] = 0;
+    for (int i = 0; i < n; ++i)
+        for (int j = 0; j < n; ++j) {
+            if (j == i) continue;
+            float dx = x[3 * i] - x[3 * j];
+            float dy = x[3 * i + 1] - x[3 * j + 1];
+            float dz = x[3 * i + 2] - x[3 * j + 2];
+            float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+            float t = sqrtf(r2) * inv_dr;
+            if (t < (float)n_bins) hist[(int)t] += 1;
+        }
+}
+
+/* Eq. 8 numerator psi(r_sun) per shell around the droplet centre, the sums of Eq. 3-4
+ * (sum x, sum |x|^2, fp64 from the fp32 state) and N_surf: NPs whose surface is
+ * within one NP radius of the interface, |x| > R - 2 r_a, decided in fp64. */
+void lvo_radial_hist(int n, const float *x, const int32_t *type, const double *radius_a,
+                     double R, float inv_dr, int n_bins, uint64_t *hist, double sums[4],
+                     int64_t *n_surf)
+{
+    for (int b = 0; b < n_bins; ++b) hist[b] = 0;
+    sums[0] = sums[1] = sums[2] = sums[3] = 0.0;
+    *n_surf = 0;
+    for (int i = 0; i < n; ++i) {
+        float fx = x[3 * i], fy = x[3 * i + 1], fz = x[3 * i + 2];
+        float t = sqrtf(fmaf(fz, fz, fmaf(fy, fy, fx * fx))) * inv_dr;
+        if (t < (float)n_bins) hist[(int)t] += 1;
+        double dx = fx, dy = fy, dz = fz;
+        double r2 = dx * dx + dy * dy + dz * dz;
+        sums[0] += dx; sums[1] += dy; sums[2] += dz; sums[3] += r2;
+        if (sqrt(r2) > R - 2.0 * radius_a[type[i]]) *n_surf += 1;
+    }
+}
+
 int lvo_sizeof_params(void) { return (int)sizeof(lvo_params); }
 int lvo_sizeof_grid(void) { return (int)sizeof(lvo_grid); }
 int lvo_max_threads(void)

@@ -30,7 +30,7 @@ FORCE_SIMPLE, FORCE_QUEUED, FORCE_SEGMENTS, FORCE_PACKED = 0, 1, 2, 3
 # every symbol include/lv.h declares (tests check the library exports them all)
 SYMBOLS = ["lv_langevin_coeffs", "lv_create", "lv_set_types", "lv_set_forces",
            "lv_set_droplet_schedule", "lv_set_grid", "lv_set_option", "lv_set_neighbour_list",
-           "lv_get_rebuild_count", "lv_workspace_bytes", "lv_bind",
+           "lv_get_rebuild_count", "lv_observe_rdf", "lv_observe_radial", "lv_workspace_bytes", "lv_bind",
            "lv_set_state", "lv_step", "lv_compute_forces", "lv_get_state", "lv_get_forces",
            "lv_get_status", "lv_get_debug", "lv_launches_per_step", "lv_step_profiled",
            "lv_stage_timing", "lv_read_stage_timing",
@@ -77,6 +77,9 @@ def load():
     L.lv_set_option.argtypes = [vp, C.c_int, C.c_int]
     L.lv_set_neighbour_list.argtypes = [vp, C.c_double, C.c_int]
     L.lv_get_rebuild_count.argtypes = [vp, C.POINTER(C.c_int64)]
+    L.lv_observe_rdf.argtypes = [vp, C.c_double, C.c_int, C.POINTER(C.c_uint64), dp]
+    L.lv_observe_radial.argtypes = [vp, C.c_double, C.c_int, C.POINTER(C.c_uint64), dp, dp, dp, dp,
+                                    C.POINTER(C.c_int64)]
     L.lv_workspace_bytes.argtypes = [vp]
     L.lv_workspace_bytes.restype = C.c_size_t
     L.lv_bind.argtypes = [vp, vp, C.c_size_t, vp]
@@ -255,6 +258,29 @@ class Simulation:
         cnt = np.empty((self.n,), dtype=np.int32)
         self._check(self.L.lv_get_forces(self.h, F.ctypes.data, cnt.ctypes.data, 0), "lv_get_forces")
         return F, cnt
+
+    def observe_rdf(self, dr: float, n_bins: int):
+        """-> (ordered-pair counts uint64[n_bins], g[n_bins]) of Eq. 6."""
+        h = np.zeros(int(n_bins), dtype=np.uint64)
+        g = np.zeros(int(n_bins))
+        self._check(self.L.lv_observe_rdf(self.h, float(dr), int(n_bins),
+                                          h.ctypes.data_as(C.POINTER(C.c_uint64)),
+                                          g.ctypes.data_as(C.POINTER(C.c_double))), "lv_observe_rdf")
+        return h, g
+
+    def observe_radial(self, dr: float, n_bins: int):
+        """-> dict(hist, conc (Eq. 8), centre (Eq. 4), r_g (Eq. 3), d_f (Eq. 2), n_surf)."""
+        h = np.zeros(int(n_bins), dtype=np.uint64)
+        c = np.zeros(int(n_bins))
+        ctr = np.zeros(3)
+        rg, df, ns = C.c_double(), C.c_double(), C.c_int64()
+        self._check(self.L.lv_observe_radial(self.h, float(dr), int(n_bins),
+                                             h.ctypes.data_as(C.POINTER(C.c_uint64)),
+                                             c.ctypes.data_as(C.POINTER(C.c_double)),
+                                             ctr.ctypes.data_as(C.POINTER(C.c_double)),
+                                             C.byref(rg), C.byref(df), C.byref(ns)),
+                    "lv_observe_radial")
+        return dict(hist=h, conc=c, centre=ctr, r_g=rg.value, d_f=df.value, n_surf=int(ns.value))
 
     def status(self) -> int:
         s = C.c_uint32()

@@ -590,6 +590,110 @@ int lv_compute_forces(lv_sim *s)
     return enqueue_rebuild_and_forces(s);
 }
 
+namespace {
+constexpr int kMaxObsBins = 8192;
+
+// scratch for the observables: the host-transfer staging area (28 n bytes)
+int obs_scratch(lv_sim *s, int n_bins, unsigned long long **hist, double **sums)
+{
+    const size_t need = 8 * (size_t)n_bins + 64;
+    if (need > 28 * (size_t)(s->n > 0 ? s->n : 1)) return LV_E_ARG;
+    *hist = (unsigned long long *)s->bufs.staging;
+    *sums = (double *)(s->bufs.staging + 8 * (size_t)n_bins);
+    LV_CUDA(s, cudaMemsetAsync(s->bufs.staging, 0, need, s->stream));
+    return LV_OK;
+}
+
+double shell_volume(int k, double dr)
+{
+    const double a = k * dr, b = (k + 1) * dr;
+    return 4.0 / 3.0 * M_PI * (b * b * b - a * a * a);
+}
+}  // namespace
+
+int lv_observe_rdf(lv_sim *s, double dr, int n_bins, uint64_t *hist, double *g)
+{
+    if (!s || !(dr > 0.0) || n_bins < 1 || n_bins > kMaxObsBins) return LV_E_ARG;
+    if (!s->bound || !s->state_set) return LV_E_ORDER;
+    if (hist) memset(hist, 0, 8 * (size_t)n_bins);
+    if (g) for (int k = 0; k < n_bins; ++k) g[k] = 0.0;
+    if (s->n == 0) return LV_OK;
+    // cell structures of the current state (steps (i) of PAPER.md:64), then the pair walk
+    for (int k = 0; k < 3; ++k) {
+        int rc = enqueue_stage(s, k);
+        if (rc != LV_OK) return rc;
+    }
+    s->force_order_b = true;
+    unsigned long long *dh = nullptr;
+    double *ds = nullptr;
+    int rc = obs_scratch(s, n_bins, &dh, &ds);
+    if (rc != LV_OK) return rc;
+    LV_CUDA(s, lvk_rdf_hist(s->dev, s->bufs, s->grid.h, dr, n_bins, dh, s->stream));
+    uint64_t *hh = (uint64_t *)malloc(8 * (size_t)n_bins);
+    if (!hh) return LV_E_NOMEM;
+    cudaError_t e = cudaMemcpyAsync(hh, dh, 8 * (size_t)n_bins, cudaMemcpyDeviceToHost, s->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s->stream);
+    if (e != cudaSuccess) { free(hh); return cuda_fail(s, e, "lv_observe_rdf"); }
+    LvDevState st;
+    e = cudaMemcpy(&st, s->bufs.st, sizeof(st), cudaMemcpyDeviceToHost);
+    if (e != cudaSuccess) { free(hh); return cuda_fail(s, e, "lv_observe_rdf"); }
+    // Eq. 6: g_k = (psi_k / N) / ((N - 1) dV_k / V), V the droplet volume at this step
+    const double R = lv_radius_of(s->sched_mode, s->R0, s->R1, s->sched_steps, st.step);
+    const double V = 4.0 / 3.0 * M_PI * R * R * R, N = (double)s->n;
+    for (int k = 0; k < n_bins; ++k) {
+        if (hist) hist[k] = hh[k];
+        if (g && s->n > 1) g[k] = ((double)hh[k] / N) / ((N - 1.0) * shell_volume(k, dr) / V);
+    }
+    free(hh);
+    return LV_OK;
+}
+
+int lv_observe_radial(lv_sim *s, double dr, int n_bins, uint64_t *hist, double *conc, double *centre,
+                      double *r_g, double *d_f, int64_t *n_surf)
+{
+    if (!s || !(dr > 0.0) || n_bins < 1 || n_bins > kMaxObsBins) return LV_E_ARG;
+    if (!s->bound || !s->state_set) return LV_E_ORDER;
+    if (hist) memset(hist, 0, 8 * (size_t)n_bins);
+    if (conc) for (int k = 0; k < n_bins; ++k) conc[k] = 0.0;
+    if (centre) centre[0] = centre[1] = centre[2] = 0.0;
+    if (r_g) *r_g = 0.0;
+    if (d_f) *d_f = 0.0;
+    if (n_surf) *n_surf = 0;
+    if (s->n == 0) return LV_OK;
+    LvDevState st;
+    LV_CUDA(s, cudaMemcpyAsync(&st, s->bufs.st, sizeof(st), cudaMemcpyDeviceToHost, s->stream));
+    LV_CUDA(s, cudaStreamSynchronize(s->stream));
+    const double R = lv_radius_of(s->sched_mode, s->R0, s->R1, s->sched_steps, st.step);
+    unsigned long long *dh = nullptr;
+    double *ds = nullptr;
+    int rc = obs_scratch(s, n_bins, &dh, &ds);
+    if (rc != LV_OK) return rc;
+    LV_CUDA(s, lvk_radial_hist(s->dev, s->bufs, s->grid.h, R, dr, n_bins, dh, ds, s->stream));
+    const size_t bytes = 8 * (size_t)n_bins + 64;
+    unsigned char *hb = (unsigned char *)malloc(bytes);
+    if (!hb) return LV_E_NOMEM;
+    cudaError_t e = cudaMemcpyAsync(hb, dh, bytes, cudaMemcpyDeviceToHost, s->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s->stream);
+    if (e != cudaSuccess) { free(hb); return cuda_fail(s, e, "lv_observe_radial"); }
+    const uint64_t *hh = (const uint64_t *)hb;
+    const double *sm = (const double *)(hb + 8 * (size_t)n_bins);
+    const double N = (double)s->n, V = 4.0 / 3.0 * M_PI * R * R * R;
+    for (int k = 0; k < n_bins; ++k) {
+        if (hist) hist[k] = hh[k];
+        if (conc) conc[k] = ((double)hh[k] / N) / (shell_volume(k, dr) / V);      // Eq. 8
+    }
+    const double cx = sm[0] / N, cy = sm[1] / N, cz = sm[2] / N;                  // Eq. 4
+    const double rg2 = sm[3] / N - (cx * cx + cy * cy + cz * cz);                 // Eq. 3
+    const double rg = rg2 > 0.0 ? sqrt(rg2) : 0.0;
+    if (centre) { centre[0] = cx; centre[1] = cy; centre[2] = cz; }
+    if (r_g) *r_g = rg;
+    // Eq. 2 solved for D_f with k_f = 1.593 and d_NP the mean NP diameter
+    if (d_f && rg > 0.0) *d_f = log(N / 1.593) / log(2.0 * rg / (sm[4] / N));
+    if (n_surf) memcpy(n_surf, sm + 5, 8);
+    free(hb);
+    return LV_OK;
+}
+
 int lv_get_status(lv_sim *s, uint32_t *status)
 {
     if (!s || !status) return LV_E_ARG;

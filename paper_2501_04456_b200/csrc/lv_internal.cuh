@@ -140,5 +140,12 @@ cudaError_t lvs_sort_pairs(void *temp, size_t temp_bytes, const uint32_t *key_in
                            const uint32_t *val_in, uint32_t *val_out, int n, int end_bit,
                            cudaStream_t st);
 
+// observables (lv_observe_*): integer histograms + fp64 sums into caller-zeroed device memory;
+// h_grid = cell edge per type grid (host)
+cudaError_t lvk_rdf_hist(const LvDev &P, const LvBufs &B, const double *h_grid, double dr, int n_bins,
+                         unsigned long long *hist, cudaStream_t st);
+cudaError_t lvk_radial_hist(const LvDev &P, const LvBufs &B, const double *h_grid, double R, double dr,
+                            int n_bins, unsigned long long *hist, double *sums, cudaStream_t st);
+
 // FP32 FMA throughput probe (lv_measure_fp32_peak)
 cudaError_t lvk_fma_peak(float *scratch, int blocks, int iters, double *flops, cudaStream_t st);

@@ -10,6 +10,9 @@
 // bits), float4 vel = (vx, vy, vz, id bits), 16-byte aligned SoA.
 #include "lv_internal.cuh"
 
+#include <cstring>
+#include <cmath>
+
 namespace {
 
 constexpr int kThreads = 128;
@@ -1121,6 +1124,103 @@ k_ids_sorted(int n, const float4 *__restrict__ velB, uint32_t *__restrict__ ids)
     if (i < n) ids[i] = __float_as_uint(velB[i].w);
 }
 
+// ------------------------------------------- observables
+// fp32 contract #4: the shell of a distance is (int) fl32(sqrt_rn(r2) * inv_dr)
+// with r2 as in contract #2; counted iff < n_bins.  Both sides evaluate exactly this.
+struct LvObs {
+    float inv_dr;
+    float r2_max;          // pre-filter only: (n_bins dr)^2 (1 + 1e-5)
+    int32_t n_bins;
+    int8_t w[LV_MAX_TYPES];   // stencil half-width on grid b for r_max
+};
+
+// Eq. 6 numerator: ordered pairs per shell.  One thread per cell-sorted NP, the cell
+// walk of the first force kernel with r_max in place of the cut-offs; counts go to a
+// per-block histogram in shared memory, then to the global one.
+__global__ void __launch_bounds__(kThreads)
+k_rdf_hist(const __grid_constant__ LvDev P, const LvObs O, const float4 *__restrict__ pos,
+           const uint32_t *__restrict__ off, unsigned long long *__restrict__ hist)
+{
+    extern __shared__ uint32_t s_hist[];
+    for (int b = threadIdx.x; b < O.n_bins; b += kThreads) s_hist[b] = 0u;
+    __syncthreads();
+    const int i = blockIdx.x * kThreads + threadIdx.x;
+    if (i < P.n) {
+        const float4 pi = pos[i];
+        const float nb = (float)O.n_bins;
+        for (int b = 0; b < P.n_types; ++b) {
+            const LvGridDev g = P.grid[b];
+            const int w = O.w[b];
+            const int cx = cell_coord(pi.x, g.lo, g.inv_h, g.G);
+            const int cy = cell_coord(pi.y, g.lo, g.inv_h, g.G);
+            const int cz = cell_coord(pi.z, g.lo, g.inv_h, g.G);
+            const int x0 = max(cx - w, 0), x1 = min(cx + w, g.G - 1);
+            const int y0 = max(cy - w, 0), y1 = min(cy + w, g.G - 1);
+            const int z0 = max(cz - w, 0), z1 = min(cz + w, g.G - 1);
+            for (int z = z0; z <= z1; ++z)
+                for (int y = y0; y <= y1; ++y) {
+                    const uint32_t row = g.base + (uint32_t)((z * g.G + y) * g.G);
+                    const uint32_t js = __ldg(off + row + x0);
+                    const uint32_t je = __ldg(off + row + x1 + 1);
+                    for (uint32_t j = js; j < je; ++j) {
+                        const float4 pj = __ldg(pos + j);
+                        const float dx = __fsub_rn(pi.x, pj.x);
+                        const float dy = __fsub_rn(pi.y, pj.y);
+                        const float dz = __fsub_rn(pi.z, pj.z);
+                        const float r2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
+                        if (r2 < O.r2_max && j != (uint32_t)i) {
+                            const float t = __fmul_rn(__fsqrt_rn(r2), O.inv_dr);
+                            if (t < nb) atomicAdd(&s_hist[(int)t], 1u);
+                        }
+                    }
+                }
+        }
+    }
+    __syncthreads();
+    for (int b = threadIdx.x; b < O.n_bins; b += kThreads)
+        if (s_hist[b]) atomicAdd(hist + b, (unsigned long long)s_hist[b]);
+}
+
+// Eq. 8 numerator (NPs per shell around the droplet centre), the sums of Eq. 3-4 in fp64
+// (sum x, sum y, sum z, sum |x|^2, sum sigma) and N_surf (|x| > R - 2 r_a, fp64).
+// sums[0..4] doubles, then N_surf as a 64-bit integer in sums[5].
+__global__ void __launch_bounds__(kThreads)
+k_radial_hist(const __grid_constant__ LvDev P, const LvObs O, const float4 *__restrict__ pos,
+              double R, unsigned long long *__restrict__ hist, double *__restrict__ sums)
+{
+    extern __shared__ uint32_t s_hist[];
+    for (int b = threadIdx.x; b < O.n_bins; b += kThreads) s_hist[b] = 0u;
+    __syncthreads();
+    const int i = blockIdx.x * kThreads + threadIdx.x;
+    double v[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+    int surf = 0;
+    if (i < P.n) {
+        const float4 p = pos[i];
+        const int a = __float_as_int(p.w);
+        const float t = __fmul_rn(__fsqrt_rn(__fmaf_rn(p.z, p.z, __fmaf_rn(p.y, p.y, __fmul_rn(p.x, p.x)))),
+                                  O.inv_dr);
+        if (t < (float)O.n_bins) atomicAdd(&s_hist[(int)t], 1u);
+        const double x = p.x, y = p.y, z = p.z;
+        const double r2 = x * x + y * y + z * z;
+        v[0] = x; v[1] = y; v[2] = z; v[3] = r2; v[4] = 2.0 * P.radius_d[a];
+        surf = sqrt(r2) > R - 2.0 * P.radius_d[a] ? 1 : 0;
+    }
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) {
+#pragma unroll
+        for (int k = 0; k < 5; ++k) v[k] += __shfl_xor_sync(0xffffffffu, v[k], d);
+        surf += __shfl_xor_sync(0xffffffffu, surf, d);
+    }
+    if ((threadIdx.x & 31) == 0) {
+#pragma unroll
+        for (int k = 0; k < 5; ++k) atomicAdd(sums + k, v[k]);
+        if (surf) atomicAdd(reinterpret_cast<unsigned long long *>(sums + 5), (unsigned long long)surf);
+    }
+    __syncthreads();
+    for (int b = threadIdx.x; b < O.n_bins; b += kThreads)
+        if (s_hist[b]) atomicAdd(hist + b, (unsigned long long)s_hist[b]);
+}
+
 inline int blocks_for(int n) { return n > 0 ? (n + kThreads - 1) / kThreads : 1; }
 
 }  // namespace
@@ -1285,6 +1385,37 @@ cudaError_t lvk_unpack_forces(const LvDev &P, const LvBufs &B, bool order_b, flo
 cudaError_t lvk_ids_sorted(const LvDev &P, const LvBufs &B, uint32_t *ids, cudaStream_t st)
 {
     k_ids_sorted<<<blocks_for(P.n), kThreads, 0, st>>>(P.n, B.velB, ids);
+    return cudaGetLastError();
+}
+
+static LvObs make_obs(const LvDev &P, const double *h_grid, double dr, int n_bins)
+{
+    LvObs O;
+    memset(&O, 0, sizeof(O));
+    const double r_max = dr * (double)n_bins;
+    O.inv_dr = (float)(1.0 / dr);
+    O.r2_max = (float)(r_max * r_max * (1.0 + 1e-5));
+    O.n_bins = n_bins;
+    for (int b = 0; b < P.n_types; ++b) {
+        double w = ceil(r_max * (1.0 + 1.0 / 1024.0) / h_grid[b]);
+        O.w[b] = (int8_t)(w > 100.0 ? 100.0 : w);
+    }
+    return O;
+}
+
+cudaError_t lvk_rdf_hist(const LvDev &P, const LvBufs &B, const double *h_grid, double dr, int n_bins,
+                         unsigned long long *hist, cudaStream_t st)
+{
+    const LvObs O = make_obs(P, h_grid, dr, n_bins);
+    k_rdf_hist<<<blocks_for(P.n), kThreads, 4 * (size_t)n_bins, st>>>(P, O, B.posB, B.cell_off, hist);
+    return cudaGetLastError();
+}
+
+cudaError_t lvk_radial_hist(const LvDev &P, const LvBufs &B, const double *h_grid, double R, double dr,
+                            int n_bins, unsigned long long *hist, double *sums, cudaStream_t st)
+{
+    const LvObs O = make_obs(P, h_grid, dr, n_bins);
+    k_radial_hist<<<blocks_for(P.n), kThreads, 4 * (size_t)n_bins, st>>>(P, O, B.posA, R, hist, sums);
     return cudaGetLastError();
 }
 

@@ -132,3 +132,39 @@ def test_clusters_equal_library_connected_components():
     # same partition: the map label -> ref label is a bijection
     pairs = set(zip(lab.tolist(), ref.tolist()))
     assert len(pairs) == ncomp
+
+
+def test_contract_histograms_equal_the_fp64_definitions():
+    """oracle.rdf_hist / radial_hist (fp32 contract #4, the integers the CUDA path must
+    reproduce bit for bit) against observables.rdf / radial_concentration (fp64,
+    np.histogram, pinned above): the same counts except for distances that round
+    across a bin edge, and exactly the same total."""
+    import oracle
+    from paper_2501_04456_b200 import workloads as W
+    w = W.make_workload("C2", 3000)
+    x = w.pos
+    dr, nb = 0.25, 40
+    h = oracle.rdf_hist(x, dr, nb)
+    r, g = O.rdf(x.astype(np.float64), w.R0, dr, dr * nb)
+    g2 = oracle.rdf_from_hist(h, w.n, w.R0, dr)
+    # recover the fp64 counts from g and compare bin by bin
+    V = 4.0 / 3.0 * np.pi * w.R0 ** 3
+    edges = dr * np.arange(nb + 1)
+    cnt64 = np.rint(g * w.n * (w.n - 1) * O.shell_volumes(edges) / V).astype(np.int64)
+    assert h.sum() > 1e5 and h.sum() % 2 == 0                  # ordered pairs come in twos
+    assert abs(int(h.sum()) - int(cnt64.sum())) <= 4
+    assert np.max(np.abs(h.astype(np.int64) - cnt64)) <= 4     # only edge-rounding moves a pair
+    assert np.allclose(g2[4:], g[4:], rtol=2e-3, atol=0)
+    # radial profile, sums and N_surf
+    ra = 0.5 * np.asarray(w.sigma)
+    hr, sums, ns = oracle.radial_hist(x, w.type, ra, w.R0, 2.0, 30)
+    x64 = x.astype(np.float64)
+    rr = np.sqrt((x64 * x64).sum(axis=1))
+    ref = np.histogram(rr, bins=2.0 * np.arange(31))[0]
+    assert hr.sum() == w.n and np.max(np.abs(hr.astype(np.int64) - ref)) <= 2
+    assert np.allclose(sums[:3], x64.sum(axis=0), rtol=0, atol=1e-9)
+    assert sums[3] == pytest.approx((rr * rr).sum(), rel=1e-13)
+    assert ns == int(np.count_nonzero(rr > w.R0 - 2.0 * ra[w.type]))
+    # R_g from the sums (Eq. 3-4): <|x|^2> - |r_0|^2
+    rg = np.sqrt(sums[3] / w.n - ((sums[:3] / w.n) ** 2).sum())
+    assert rg == pytest.approx(O.radius_of_gyration(x64), rel=1e-12)
