@@ -259,6 +259,34 @@ def run_lv(args):
         }
         vs.close()
 
+    # ---- NEXT-1 rows: the paper's observables on the device (synchronous calls) -------
+    observables = {}
+    if rank == 0 and world == 1 and not args.no_variants:
+        nb = 100
+        drb = 5.0 / nb                                  # g(r) to r = 5 sigma, as in the long-run tests
+        sim.observe_rdf(drb, nb); sim.observe_radial(w.R0 / 100.0, 128)      # warm
+        t0 = time.perf_counter()
+        for _ in range(5):
+            hh, _ = sim.observe_rdf(drb, nb)
+        t_rdf = (time.perf_counter() - t0) / 5
+        t0 = time.perf_counter()
+        for _ in range(5):
+            sim.observe_radial(w.R0 / 100.0, 128)
+        t_rad = (time.perf_counter() - t0) / 5
+        t0 = time.perf_counter()
+        for _ in range(5):
+            cl = sim.observe_clusters(1.5, want_labels=False)
+        t_cl = (time.perf_counter() - t0) / 5
+        observables = {
+            "clusters": {"ms": t_cl * 1e3, "bond_factor": 1.5, "n_clusters": cl["n_clusters"],
+                         "largest": cl["largest"],
+                         "how": "lv_observe_clusters: cell rebuild + union-find + statistics, wall clock"},
+            "rdf": {"ms": t_rdf * 1e3, "bins": nb, "dr": drb, "ordered_pairs": int(hh.sum()),
+                    "how": "lv_observe_rdf: cell rebuild + pair walk + D2H of the histogram, wall clock"},
+            "radial": {"ms": t_rad * 1e3, "bins": 128,
+                       "how": "lv_observe_radial: one pass over the NPs + D2H, wall clock"},
+        }
+
     # ---- e2e: host buffers through the C ABI, copies inside the timed region
     n = w.n
     hp = torch.empty((n, 3), dtype=torch.float32).pin_memory()
@@ -328,6 +356,7 @@ def run_lv(args):
         "wall_s_timed_region": wall_s,
         "roofline": roofline,
         "variants": variants,
+        "observables": observables,
         "resident": {"value": float(n) * args.steps * world / (res_max * 1e-3), "unit": UNIT,
                      "ms_per_step": res_max / args.steps,
                      "how": "lv_step(K) as CUDA-graph replay, no L2 flush, events around the K steps"},

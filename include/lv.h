@@ -238,6 +238,18 @@ int lv_observe_rdf(lv_sim *s, double dr, int n_bins, uint64_t *hist, double *g);
 int lv_observe_radial(lv_sim *s, double dr, int n_bins, uint64_t *hist, double *conc,
                       double *centre, double *r_g, double *d_f, int64_t *n_surf);
 
+/* lv_observe_clusters: aggregates ("aggregate statistics",
+ * "number of sub-aggregates", PAPER.md:58 -- not defined there, reading R23): connected
+ * components of the graph whose edges are the pairs with r2 < fl32((bond_factor
+ * sigma_ab)^2), r2 as in the in-range predicate.  bond_factor sigma_ab must not exceed
+ * r_c,ab (LV_E_ARG).  labels: host int32[n] by NP id, the label of an NP is the smallest
+ * NP id of its aggregate; n_clusters, largest (NPs in the largest aggregate), mean_size
+ * = n / n_clusters; log2_hist: host uint64[32], aggregates with size in [2^k, 2^(k+1)).
+ * All written, any may be NULL.  Rebuilds the cell structures; synchronises; the state
+ * does not change. */
+int lv_observe_clusters(lv_sim *s, double bond_factor, int32_t *labels, int64_t *n_clusters,
+                        double *mean_size, int64_t *largest, uint64_t *log2_hist);
+
 /* Status bits LV_ST_* (host uint32, written).  Synchronises. */
 int lv_get_status(lv_sim *s, uint32_t *status);
 

@@ -94,6 +94,8 @@ def lib():
         L.lvo_radial_hist.argtypes = [C.c_int, fp, ip, dp, C.c_double, C.c_float, C.c_int,
                                       C.POINTER(C.c_uint64), dp, C.POINTER(C.c_int64)]
         L.lvo_radial_hist.restype = None
+        L.lvo_cluster_labels.argtypes = [C.c_int, fp, ip, fp, ip]
+        L.lvo_cluster_labels.restype = None
         L.lvo_sizeof_params.restype = C.c_int
         L.lvo_sizeof_grid.restype = C.c_int
         L.lvo_max_threads.restype = C.c_int
@@ -323,3 +325,17 @@ def rdf_from_hist(hist, n, R, dr):
     dV = 4.0 / 3.0 * np.pi * (((k + 1) * dr) ** 3 - (k * dr) ** 3)
     V = 4.0 / 3.0 * np.pi * float(R) ** 3
     return (np.asarray(hist, dtype=np.float64) / n) / ((n - 1) * dV / V)
+
+
+def cluster_labels(x_f32, type_, sigma_ab, bond_factor=1.5):
+    """Aggregates with the bond predicate in fp32 (contract #2 with (bond_factor sigma_ab)^2):
+    label[i] = smallest index of i's connected component.  sigma_ab: T x T."""
+    x = np.ascontiguousarray(x_f32, dtype=np.float32).reshape(-1, 3)
+    t = _ci32(type_)
+    sg = np.asarray(sigma_ab, dtype=np.float64)
+    rb2 = np.zeros((MAX_TYPES, MAX_TYPES), dtype=np.float32)
+    T = sg.shape[0]
+    rb2[:T, :T] = ((bond_factor * sg) ** 2).astype(np.float32)
+    lab = np.zeros(x.shape[0], dtype=np.int32)
+    lib().lvo_cluster_labels(x.shape[0], _f(x), _i(t), _f(rb2), _i(lab))
+    return lab

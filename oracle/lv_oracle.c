@@ -572,6 +572,28 @@ void lvo_radial_hist(int n, const float *x, const int32_t *type, const double *r
     }
 }
 
+/* Aggregates (reading R23): connected components of the bond graph r2 < rb2_ab, r2 by
+ * contract #2 on the fp32 state, rb2 a T x T fp32 table (row stride LVO_MAX_TYPES) of
+ * squared bond lengths.  Plain O(N^2) union by relabelling: label[i] = smallest index of
+ * i's component. */
+void lvo_cluster_labels(int n, const float *x, const int32_t *type, const float *rb2,
+                        int32_t *label)
+{
+    for (int i = 0; i < n; ++i) label[i] = i;
+    int changed = 1;
+    while (changed) {               /* propagate the minimum label along bonds until stable */
+        changed = 0;
+        for (int i = 0; i < n; ++i)
+            for (int j = 0; j < n; ++j) {
+                if (j == i || label[j] >= label[i]) continue;
+                if (in_range_f32(x + 3 * i, x + 3 * j, rb2[type[i] * LVO_MAX_TYPES + type[j]])) {
+                    label[i] = label[j];
+                    changed = 1;
+                }
+            }
+    }
+}
+
 int lvo_sizeof_params(void) { return (int)sizeof(lvo_params); }
 int lvo_sizeof_grid(void) { return (int)sizeof(lvo_grid); }
 int lvo_max_threads(void)

@@ -30,7 +30,7 @@ FORCE_SIMPLE, FORCE_QUEUED, FORCE_SEGMENTS, FORCE_PACKED = 0, 1, 2, 3
 # every symbol include/lv.h declares (tests check the library exports them all)
 SYMBOLS = ["lv_langevin_coeffs", "lv_create", "lv_set_types", "lv_set_forces",
            "lv_set_droplet_schedule", "lv_set_grid", "lv_set_option", "lv_set_neighbour_list",
-           "lv_get_rebuild_count", "lv_observe_rdf", "lv_observe_radial", "lv_workspace_bytes", "lv_bind",
+           "lv_get_rebuild_count", "lv_observe_rdf", "lv_observe_radial", "lv_observe_clusters", "lv_workspace_bytes", "lv_bind",
            "lv_set_state", "lv_step", "lv_compute_forces", "lv_get_state", "lv_get_forces",
            "lv_get_status", "lv_get_debug", "lv_launches_per_step", "lv_step_profiled",
            "lv_stage_timing", "lv_read_stage_timing",
@@ -78,6 +78,8 @@ def load():
     L.lv_set_neighbour_list.argtypes = [vp, C.c_double, C.c_int]
     L.lv_get_rebuild_count.argtypes = [vp, C.POINTER(C.c_int64)]
     L.lv_observe_rdf.argtypes = [vp, C.c_double, C.c_int, C.POINTER(C.c_uint64), dp]
+    L.lv_observe_clusters.argtypes = [vp, C.c_double, ip, C.POINTER(C.c_int64), dp,
+                                      C.POINTER(C.c_int64), C.POINTER(C.c_uint64)]
     L.lv_observe_radial.argtypes = [vp, C.c_double, C.c_int, C.POINTER(C.c_uint64), dp, dp, dp, dp,
                                     C.POINTER(C.c_int64)]
     L.lv_workspace_bytes.argtypes = [vp]
@@ -281,6 +283,20 @@ class Simulation:
                                              C.byref(rg), C.byref(df), C.byref(ns)),
                     "lv_observe_radial")
         return dict(hist=h, conc=c, centre=ctr, r_g=rg.value, d_f=df.value, n_surf=int(ns.value))
+
+    def observe_clusters(self, bond_factor: float = 1.5, want_labels: bool = True):
+        """-> dict(labels int32[n] by id (smallest id of the aggregate) or None, n_clusters,
+        mean_size, largest, log2_hist uint64[32])."""
+        lab = np.zeros(self.n, dtype=np.int32) if want_labels else None
+        nc, lg, ms = C.c_int64(), C.c_int64(), C.c_double()
+        hist = np.zeros(32, dtype=np.uint64)
+        self._check(self.L.lv_observe_clusters(
+            self.h, float(bond_factor),
+            lab.ctypes.data_as(C.POINTER(C.c_int32)) if want_labels else None,
+            C.byref(nc), C.byref(ms), C.byref(lg), hist.ctypes.data_as(C.POINTER(C.c_uint64))),
+            "lv_observe_clusters")
+        return dict(labels=lab, n_clusters=int(nc.value), mean_size=ms.value, largest=int(lg.value),
+                    log2_hist=hist)
 
     def status(self) -> int:
         s = C.c_uint32()

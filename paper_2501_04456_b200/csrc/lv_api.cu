@@ -694,6 +694,50 @@ int lv_observe_radial(lv_sim *s, double dr, int n_bins, uint64_t *hist, double *
     return LV_OK;
 }
 
+int lv_observe_clusters(lv_sim *s, double bond_factor, int32_t *labels, int64_t *n_clusters,
+                        double *mean_size, int64_t *largest, uint64_t *log2_hist)
+{
+    if (!s || !(bond_factor > 0.0)) return LV_E_ARG;
+    if (!s->bound || !s->state_set) return LV_E_ORDER;
+    if (n_clusters) *n_clusters = 0;
+    if (mean_size) *mean_size = 0.0;
+    if (largest) *largest = 0;
+    if (log2_hist) memset(log2_hist, 0, 8 * 32);
+    if (s->n == 0) return LV_OK;
+    const int T = s->n_types;
+    float rb2[LV_MAX_TYPES * LV_MAX_TYPES];
+    memset(rb2, 0, sizeof(rb2));
+    for (int a = 0; a < T; ++a)
+        for (int b = 0; b < T; ++b) {
+            const int k = a * LV_MAX_TYPES + b;
+            const double rb = bond_factor * s->sig[k];
+            if (rb > s->rcut[k]) return LV_E_ARG;      // bonds are searched inside the force stencil
+            rb2[k] = (float)(rb * rb);
+        }
+    for (int k = 0; k < 3; ++k) {                      // cell structures of the current state
+        int rc = enqueue_stage(s, k);
+        if (rc != LV_OK) return rc;
+    }
+    s->force_order_b = true;
+    // scratch in the staging area: 3 uint32[n] | int32 labels[n] | 34 u64 statistics
+    const size_t n = (size_t)s->n;
+    if (28 * n < 16 * n + 34 * 8 + 8) return LV_E_ARG;
+    uint32_t *scratch = (uint32_t *)s->bufs.staging;
+    int32_t *dlab = (int32_t *)(s->bufs.staging + 12 * n);
+    unsigned long long *dst = (unsigned long long *)(s->bufs.staging + ((16 * n + 7) / 8) * 8);
+    LV_CUDA(s, cudaMemsetAsync(dst, 0, 34 * 8, s->stream));
+    LV_CUDA(s, lvk_clusters(s->dev, s->bufs, rb2, scratch, labels ? dlab : nullptr, dst, s->stream));
+    unsigned long long hs[34];
+    LV_CUDA(s, cudaMemcpyAsync(hs, dst, sizeof(hs), cudaMemcpyDeviceToHost, s->stream));
+    if (labels) LV_CUDA(s, cudaMemcpyAsync(labels, dlab, 4 * n, cudaMemcpyDeviceToHost, s->stream));
+    LV_CUDA(s, cudaStreamSynchronize(s->stream));
+    if (n_clusters) *n_clusters = (int64_t)hs[0];
+    if (largest) *largest = (int64_t)hs[1];
+    if (mean_size && hs[0] > 0) *mean_size = (double)n / (double)hs[0];
+    if (log2_hist) for (int k = 0; k < 32; ++k) log2_hist[k] = hs[2 + k];
+    return LV_OK;
+}
+
 int lv_get_status(lv_sim *s, uint32_t *status)
 {
     if (!s || !status) return LV_E_ARG;

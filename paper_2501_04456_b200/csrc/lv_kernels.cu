@@ -1221,6 +1221,112 @@ k_radial_hist(const __grid_constant__ LvDev P, const LvObs O, const float4 *__re
         if (s_hist[b]) atomicAdd(hist + b, (unsigned long long)s_hist[b]);
 }
 
+// ---------------------------------- aggregates (reading R23)
+// Connected components of the bond graph r_ij < bond_factor * sigma_ab, by lock-free
+// union-find over cell-sorted slots: every NP hooks itself to each bonded neighbour with a
+// smaller slot (atomicMin on the larger root), then every slot is compressed to its root.
+// The bond predicate is contract #2 with rb2_ab in place of r_c,ab^2.
+struct LvBond {
+    float rb2[LV_MAX_TYPES * LV_MAX_TYPES];
+};
+
+__device__ __forceinline__ uint32_t cc_find(uint32_t *parent, uint32_t a)
+{
+    // volatile: other blocks re-hook roots while we walk; always read through to L2
+    volatile uint32_t *vp = parent;
+    uint32_t p = vp[a];
+    while (p != a) {
+        const uint32_t gp = vp[p];
+        if (gp != p) parent[a] = gp;        // path halving (benign race: any ancestor is valid)
+        a = p;
+        p = gp;
+    }
+    return a;
+}
+
+__global__ void __launch_bounds__(kThreads) k_cc_init(int n, uint32_t *parent, uint32_t *min_id,
+                                                      uint32_t *size)
+{
+    const int i = blockIdx.x * kThreads + threadIdx.x;
+    if (i < n) { parent[i] = (uint32_t)i; min_id[i] = 0xffffffffu; size[i] = 0u; }
+}
+
+__global__ void __launch_bounds__(kThreads)
+k_cc_hook(const __grid_constant__ LvDev P, const LvBond Bd, const float4 *__restrict__ pos,
+          const uint32_t *__restrict__ off, uint32_t *parent)
+{
+    const int i = blockIdx.x * kThreads + threadIdx.x;
+    if (i >= P.n) return;
+    const float4 pi = pos[i];
+    const int a = __float_as_int(pi.w);
+    for (int b = 0; b < P.n_types; ++b) {
+        const LvGridDev g = P.grid[b];
+        const int w = P.w[a * LV_MAX_TYPES + b];
+        const float rb2 = Bd.rb2[a * LV_MAX_TYPES + b];
+        const int cx = cell_coord(pi.x, g.lo, g.inv_h, g.G);
+        const int cy = cell_coord(pi.y, g.lo, g.inv_h, g.G);
+        const int cz = cell_coord(pi.z, g.lo, g.inv_h, g.G);
+        const int x0 = max(cx - w, 0), x1 = min(cx + w, g.G - 1);
+        const int y0 = max(cy - w, 0), y1 = min(cy + w, g.G - 1);
+        const int z0 = max(cz - w, 0), z1 = min(cz + w, g.G - 1);
+        for (int z = z0; z <= z1; ++z)
+            for (int y = y0; y <= y1; ++y) {
+                const uint32_t row = g.base + (uint32_t)((z * g.G + y) * g.G);
+                const uint32_t js = __ldg(off + row + x0);
+                uint32_t je = __ldg(off + row + x1 + 1);
+                if (je > (uint32_t)i) je = (uint32_t)i;          // each bond once: j < i
+                for (uint32_t j = js; j < je; ++j) {
+                    const float4 pj = pos[j];
+                    const float dx = __fsub_rn(pi.x, pj.x);
+                    const float dy = __fsub_rn(pi.y, pj.y);
+                    const float dz = __fsub_rn(pi.z, pj.z);
+                    const float r2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
+                    if (r2 < rb2) {
+                        uint32_t u = cc_find(parent, (uint32_t)i), v = cc_find(parent, j);
+                        while (u != v) {
+                            if (u < v) { const uint32_t t = u; u = v; v = t; }    // hook larger under smaller
+                            const uint32_t old = atomicMin(parent + u, v);
+                            if (old == u) break;
+                            u = cc_find(parent, old);
+                            v = cc_find(parent, v);
+                        }
+                    }
+                }
+            }
+    }
+}
+
+// root of every slot; per root: smallest NP id and number of members
+__global__ void __launch_bounds__(kThreads)
+k_cc_roots(int n, uint32_t *parent, const float4 *__restrict__ vel, uint32_t *min_id, uint32_t *size)
+{
+    const int i = blockIdx.x * kThreads + threadIdx.x;
+    if (i >= n) return;
+    const uint32_t r = cc_find(parent, (uint32_t)i);
+    parent[i] = r;
+    atomicMin(min_id + r, __float_as_uint(vel[i].w));
+    atomicAdd(size + r, 1u);
+}
+
+// label of an NP = smallest NP id of its aggregate (unique, order-free); statistics per root:
+// stats[0] = aggregates, stats[1] = largest, stats[2 + k] = aggregates of size in [2^k, 2^(k+1))
+__global__ void __launch_bounds__(kThreads)
+k_cc_labels(int n, const uint32_t *__restrict__ parent, const float4 *__restrict__ vel,
+            const uint32_t *__restrict__ min_id, const uint32_t *__restrict__ size,
+            int32_t *__restrict__ label_by_id, unsigned long long *stats)
+{
+    const int i = blockIdx.x * kThreads + threadIdx.x;
+    if (i >= n) return;
+    const uint32_t r = parent[i];
+    if (label_by_id) label_by_id[__float_as_uint(vel[i].w)] = (int32_t)min_id[r];
+    if (r == (uint32_t)i) {
+        const uint32_t s = size[i];
+        atomicAdd(stats, 1ull);
+        atomicMax(stats + 1, (unsigned long long)s);
+        atomicAdd(stats + 2 + (31 - __clz(s)), 1ull);
+    }
+}
+
 inline int blocks_for(int n) { return n > 0 ? (n + kThreads - 1) / kThreads : 1; }
 
 }  // namespace
@@ -1416,6 +1522,21 @@ cudaError_t lvk_radial_hist(const LvDev &P, const LvBufs &B, const double *h_gri
 {
     const LvObs O = make_obs(P, h_grid, dr, n_bins);
     k_radial_hist<<<blocks_for(P.n), kThreads, 4 * (size_t)n_bins, st>>>(P, O, B.posA, R, hist, sums);
+    return cudaGetLastError();
+}
+
+// scratch: 3 uint32[n]; label_by_id int32[n] or null; stats 34 x u64, zeroed by the caller
+cudaError_t lvk_clusters(const LvDev &P, const LvBufs &B, const float *rb2, uint32_t *scratch,
+                         int32_t *label_by_id, unsigned long long *stats, cudaStream_t st)
+{
+    LvBond Bd;
+    memcpy(Bd.rb2, rb2, sizeof(Bd.rb2));
+    uint32_t *parent = scratch, *min_id = scratch + P.n, *size = scratch + 2 * (size_t)P.n;
+    k_cc_init<<<blocks_for(P.n), kThreads, 0, st>>>(P.n, parent, min_id, size);
+    k_cc_hook<<<blocks_for(P.n), kThreads, 0, st>>>(P, Bd, B.posB, B.cell_off, parent);
+    k_cc_roots<<<blocks_for(P.n), kThreads, 0, st>>>(P.n, parent, B.velB, min_id, size);
+    k_cc_labels<<<blocks_for(P.n), kThreads, 0, st>>>(P.n, parent, B.velB, min_id, size, label_by_id,
+                                                      stats);
     return cudaGetLastError();
 }
 

@@ -117,3 +117,39 @@ def test_argument_checks(B):
         with pytest.raises(B.LvError):
             sim.observe_radial(*bad)
     sim.close()
+
+
+@pytest.mark.parametrize("name,n,cpc,scale,steps", [
+    ("C1", None, None, 1.0, 0),
+    ("C1", None, None, 1.0, 3000),            # the LJ gas has started to condense
+    ("C2", 8191, [2, 2], 0.6, 0),             # compressed: large aggregates
+    ("C3", 20000, [1, 2, 2], 0.5, 0),
+    ("C4", 19999, [2], 1.0, 0),               # dense: one percolating aggregate + a few
+])
+def test_aggregates_equal_the_oracle_partition(B, orc, name, n, cpc, scale, steps):
+    from oracle import observables as O
+    w = W.make_workload(name, n)
+    if scale != 1.0:
+        w.pos = (w.pos * np.float32(scale)).astype(np.float32)
+    sim = B.Simulation.from_workload(w, cells_per_cut=cpc)
+    if steps:
+        sim.step(steps)
+    x, v, t, R, st = sim.get_state(check=False)
+    out = sim.observe_clusters(1.5)
+    sg = np.asarray(w.sigma)
+    lab = orc.cluster_labels(x, w.type, 0.5 * (sg[:, None] + sg[None, :]), 1.5)
+    assert np.array_equal(out["labels"], lab)                 # canonical labels: bit-exact
+    stats = O.cluster_statistics(np.unique(lab, return_inverse=True)[1])
+    assert out["n_clusters"] == stats["n_clusters"]
+    assert out["largest"] == stats["largest"]
+    assert out["mean_size"] == pytest.approx(stats["mean_size"], rel=1e-14)
+    hist = np.zeros(32, dtype=np.uint64)
+    hist[:len(stats["log2_hist"])] = stats["log2_hist"]
+    assert np.array_equal(out["log2_hist"], hist)
+    # statistics only (no label transfer) give the same numbers
+    out2 = sim.observe_clusters(1.5, want_labels=False)
+    assert out2["labels"] is None and out2["n_clusters"] == out["n_clusters"]
+    # a bond longer than the cut-off cannot be searched in the force stencil
+    with pytest.raises(B.LvError):
+        sim.observe_clusters(100.0)
+    sim.close()

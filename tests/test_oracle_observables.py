@@ -168,3 +168,23 @@ def test_contract_histograms_equal_the_fp64_definitions():
     # R_g from the sums (Eq. 3-4): <|x|^2> - |r_0|^2
     rg = np.sqrt(sums[3] / w.n - ((sums[:3] / w.n) ** 2).sum())
     assert rg == pytest.approx(O.radius_of_gyration(x64), rel=1e-12)
+
+
+def test_contract_cluster_labels_equal_the_fp64_definition():
+    """oracle.cluster_labels (fp32 bond predicate, min-label propagation in C) gives the
+    same partition as observables.cluster_labels (fp64, union-find), which is pinned to
+    scipy above."""
+    import oracle
+    from paper_2501_04456_b200 import workloads as W
+    w = W.make_workload("C2", 3000)
+    x = (w.pos * np.float32(0.6)).astype(np.float32)           # compress: plenty of bonds
+    sg = np.asarray(w.sigma)
+    sab = 0.5 * (sg[:, None] + sg[None, :])
+    lab = oracle.cluster_labels(x, w.type, sab, 1.5)
+    ref = O.cluster_labels(x.astype(np.float64), w.type, sg, 1.5)
+    assert 10 < ref.max() + 1 < w.n
+    pairs = set(zip(lab.tolist(), ref.tolist()))
+    assert len(pairs) == ref.max() + 1 == len(set(lab.tolist()))
+    # canonical: the label is the smallest member
+    for l in np.unique(lab)[:50]:
+        assert np.nonzero(lab == l)[0].min() == l
