@@ -1230,6 +1230,16 @@ struct LvBond {
     float rb2[LV_MAX_TYPES * LV_MAX_TYPES];
 };
 
+// read-only walk to the root (used once the hooking is over, where a late path-halving
+// store could overwrite the final parent[i] = root of another thread)
+__device__ __forceinline__ uint32_t cc_root(const uint32_t *parent, uint32_t a)
+{
+    const volatile uint32_t *vp = parent;
+    uint32_t p = vp[a];
+    while (p != a) { a = p; p = vp[a]; }
+    return a;
+}
+
 __device__ __forceinline__ uint32_t cc_find(uint32_t *parent, uint32_t a)
 {
     // volatile: other blocks re-hook roots while we walk; always read through to L2
@@ -1298,12 +1308,13 @@ k_cc_hook(const __grid_constant__ LvDev P, const LvBond Bd, const float4 *__rest
 
 // root of every slot; per root: smallest NP id and number of members
 __global__ void __launch_bounds__(kThreads)
-k_cc_roots(int n, uint32_t *parent, const float4 *__restrict__ vel, uint32_t *min_id, uint32_t *size)
+k_cc_roots(int n, const uint32_t *parent, uint32_t *__restrict__ root,
+           const float4 *__restrict__ vel, uint32_t *min_id, uint32_t *size)
 {
     const int i = blockIdx.x * kThreads + threadIdx.x;
     if (i >= n) return;
-    const uint32_t r = cc_find(parent, (uint32_t)i);
-    parent[i] = r;
+    const uint32_t r = cc_root(parent, (uint32_t)i);
+    root[i] = r;
     atomicMin(min_id + r, __float_as_uint(vel[i].w));
     atomicAdd(size + r, 1u);
 }
@@ -1311,13 +1322,13 @@ k_cc_roots(int n, uint32_t *parent, const float4 *__restrict__ vel, uint32_t *mi
 // label of an NP = smallest NP id of its aggregate (unique, order-free); statistics per root:
 // stats[0] = aggregates, stats[1] = largest, stats[2 + k] = aggregates of size in [2^k, 2^(k+1))
 __global__ void __launch_bounds__(kThreads)
-k_cc_labels(int n, const uint32_t *__restrict__ parent, const float4 *__restrict__ vel,
+k_cc_labels(int n, const uint32_t *__restrict__ root, const float4 *__restrict__ vel,
             const uint32_t *__restrict__ min_id, const uint32_t *__restrict__ size,
             int32_t *__restrict__ label_by_id, unsigned long long *stats)
 {
     const int i = blockIdx.x * kThreads + threadIdx.x;
     if (i >= n) return;
-    const uint32_t r = parent[i];
+    const uint32_t r = root[i];
     if (label_by_id) label_by_id[__float_as_uint(vel[i].w)] = (int32_t)min_id[r];
     if (r == (uint32_t)i) {
         const uint32_t s = size[i];
@@ -1532,10 +1543,11 @@ cudaError_t lvk_clusters(const LvDev &P, const LvBufs &B, const float *rb2, uint
     LvBond Bd;
     memcpy(Bd.rb2, rb2, sizeof(Bd.rb2));
     uint32_t *parent = scratch, *min_id = scratch + P.n, *size = scratch + 2 * (size_t)P.n;
+    uint32_t *root = B.val_in;            // free after the rebuild (arrival ranks / radix input values)
     k_cc_init<<<blocks_for(P.n), kThreads, 0, st>>>(P.n, parent, min_id, size);
     k_cc_hook<<<blocks_for(P.n), kThreads, 0, st>>>(P, Bd, B.posB, B.cell_off, parent);
-    k_cc_roots<<<blocks_for(P.n), kThreads, 0, st>>>(P.n, parent, B.velB, min_id, size);
-    k_cc_labels<<<blocks_for(P.n), kThreads, 0, st>>>(P.n, parent, B.velB, min_id, size, label_by_id,
+    k_cc_roots<<<blocks_for(P.n), kThreads, 0, st>>>(P.n, parent, root, B.velB, min_id, size);
+    k_cc_labels<<<blocks_for(P.n), kThreads, 0, st>>>(P.n, root, B.velB, min_id, size, label_by_id,
                                                       stats);
     return cudaGetLastError();
 }
