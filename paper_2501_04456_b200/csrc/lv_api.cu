@@ -726,7 +726,7 @@ int lv_observe_clusters(lv_sim *s, double bond_factor, int32_t *labels, int64_t 
     int32_t *dlab = (int32_t *)(s->bufs.staging + 12 * n);
     unsigned long long *dst = (unsigned long long *)(s->bufs.staging + ((16 * n + 7) / 8) * 8);
     LV_CUDA(s, cudaMemsetAsync(dst, 0, 34 * 8, s->stream));
-    LV_CUDA(s, lvk_clusters(s->dev, s->bufs, rb2, scratch, labels ? dlab : nullptr, dst, s->stream));
+    LV_CUDA(s, lvk_clusters(s->dev, s->bufs, rb2, s->grid.h, scratch, labels ? dlab : nullptr, dst, s->stream));
     unsigned long long hs[34];
     LV_CUDA(s, cudaMemcpyAsync(hs, dst, sizeof(hs), cudaMemcpyDeviceToHost, s->stream));
     if (labels) LV_CUDA(s, cudaMemcpyAsync(labels, dlab, 4 * n, cudaMemcpyDeviceToHost, s->stream));

@@ -148,8 +148,9 @@ cudaError_t lvk_radial_hist(const LvDev &P, const LvBufs &B, const double *h_gri
                             int n_bins, unsigned long long *hist, double *sums, cudaStream_t st);
 
 // aggregates: rb2 = T x T squared bond lengths (fp32, host); scratch 3 uint32[n] (device)
-cudaError_t lvk_clusters(const LvDev &P, const LvBufs &B, const float *rb2, uint32_t *scratch,
-                         int32_t *label_by_id, unsigned long long *stats, cudaStream_t st);
+cudaError_t lvk_clusters(const LvDev &P, const LvBufs &B, const float *rb2, const double *h_grid,
+                         uint32_t *scratch, int32_t *label_by_id, unsigned long long *stats,
+                         cudaStream_t st);
 
 // FP32 FMA throughput probe (lv_measure_fp32_peak)
 cudaError_t lvk_fma_peak(float *scratch, int blocks, int iters, double *flops, cudaStream_t st);

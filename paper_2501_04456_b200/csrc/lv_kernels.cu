@@ -1211,12 +1211,23 @@ k_radial_hist(const __grid_constant__ LvDev P, const LvObs O, const float4 *__re
         for (int k = 0; k < 5; ++k) v[k] += __shfl_xor_sync(0xffffffffu, v[k], d);
         surf += __shfl_xor_sync(0xffffffffu, surf, d);
     }
+    __shared__ double s_v[kThreads / 32][5];
+    __shared__ int s_surf[kThreads / 32];
     if ((threadIdx.x & 31) == 0) {
 #pragma unroll
-        for (int k = 0; k < 5; ++k) atomicAdd(sums + k, v[k]);
-        if (surf) atomicAdd(reinterpret_cast<unsigned long long *>(sums + 5), (unsigned long long)surf);
+        for (int k = 0; k < 5; ++k) s_v[threadIdx.x >> 5][k] = v[k];
+        s_surf[threadIdx.x >> 5] = surf;
     }
     __syncthreads();
+    if (threadIdx.x < 5) {              // one atomic per block and quantity
+        double t = 0.0;
+        for (int wq = 0; wq < kThreads / 32; ++wq) t += s_v[wq][threadIdx.x];
+        atomicAdd(sums + threadIdx.x, t);
+    } else if (threadIdx.x == 5) {
+        int t = 0;
+        for (int wq = 0; wq < kThreads / 32; ++wq) t += s_surf[wq];
+        if (t) atomicAdd(reinterpret_cast<unsigned long long *>(sums + 5), (unsigned long long)t);
+    }
     for (int b = threadIdx.x; b < O.n_bins; b += kThreads)
         if (s_hist[b]) atomicAdd(hist + b, (unsigned long long)s_hist[b]);
 }
@@ -1228,6 +1239,7 @@ k_radial_hist(const __grid_constant__ LvDev P, const LvObs O, const float4 *__re
 // The bond predicate is contract #2 with rb2_ab in place of r_c,ab^2.
 struct LvBond {
     float rb2[LV_MAX_TYPES * LV_MAX_TYPES];
+    int8_t w[LV_MAX_TYPES * LV_MAX_TYPES];    // stencil half-width on grid b for the bond length
 };
 
 // read-only walk to the root (used once the hooking is over, where a late path-halving
@@ -1271,7 +1283,7 @@ k_cc_hook(const __grid_constant__ LvDev P, const LvBond Bd, const float4 *__rest
     const int a = __float_as_int(pi.w);
     for (int b = 0; b < P.n_types; ++b) {
         const LvGridDev g = P.grid[b];
-        const int w = P.w[a * LV_MAX_TYPES + b];
+        const int w = Bd.w[a * LV_MAX_TYPES + b];
         const float rb2 = Bd.rb2[a * LV_MAX_TYPES + b];
         const int cx = cell_coord(pi.x, g.lo, g.inv_h, g.G);
         const int cy = cell_coord(pi.y, g.lo, g.inv_h, g.G);
@@ -1326,15 +1338,27 @@ k_cc_labels(int n, const uint32_t *__restrict__ root, const float4 *__restrict__
             const uint32_t *__restrict__ min_id, const uint32_t *__restrict__ size,
             int32_t *__restrict__ label_by_id, unsigned long long *stats)
 {
+    __shared__ uint32_t s_hist[32];
+    __shared__ uint32_t s_roots, s_largest;
+    if (threadIdx.x < 32) s_hist[threadIdx.x] = 0u;
+    if (threadIdx.x == 0) { s_roots = 0u; s_largest = 0u; }
+    __syncthreads();
     const int i = blockIdx.x * kThreads + threadIdx.x;
-    if (i >= n) return;
-    const uint32_t r = root[i];
-    if (label_by_id) label_by_id[__float_as_uint(vel[i].w)] = (int32_t)min_id[r];
-    if (r == (uint32_t)i) {
-        const uint32_t s = size[i];
-        atomicAdd(stats, 1ull);
-        atomicMax(stats + 1, (unsigned long long)s);
-        atomicAdd(stats + 2 + (31 - __clz(s)), 1ull);
+    if (i < n) {
+        const uint32_t r = root[i];
+        if (label_by_id) label_by_id[__float_as_uint(vel[i].w)] = (int32_t)min_id[r];
+        if (r == (uint32_t)i) {
+            const uint32_t s = size[i];
+            atomicAdd(&s_roots, 1u);
+            atomicMax(&s_largest, s);
+            atomicAdd(&s_hist[31 - __clz(s)], 1u);
+        }
+    }
+    __syncthreads();
+    if (threadIdx.x < 32 && s_hist[threadIdx.x]) atomicAdd(stats + 2 + threadIdx.x, (unsigned long long)s_hist[threadIdx.x]);
+    if (threadIdx.x == 0 && s_roots) {
+        atomicAdd(stats, (unsigned long long)s_roots);
+        atomicMax(stats + 1, (unsigned long long)s_largest);
     }
 }
 
@@ -1537,11 +1561,18 @@ cudaError_t lvk_radial_hist(const LvDev &P, const LvBufs &B, const double *h_gri
 }
 
 // scratch: 3 uint32[n]; label_by_id int32[n] or null; stats 34 x u64, zeroed by the caller
-cudaError_t lvk_clusters(const LvDev &P, const LvBufs &B, const float *rb2, uint32_t *scratch,
-                         int32_t *label_by_id, unsigned long long *stats, cudaStream_t st)
+cudaError_t lvk_clusters(const LvDev &P, const LvBufs &B, const float *rb2, const double *h_grid,
+                         uint32_t *scratch, int32_t *label_by_id, unsigned long long *stats,
+                         cudaStream_t st)
 {
     LvBond Bd;
     memcpy(Bd.rb2, rb2, sizeof(Bd.rb2));
+    for (int a = 0; a < P.n_types; ++a)
+        for (int b = 0; b < P.n_types; ++b) {
+            const int k = a * LV_MAX_TYPES + b;
+            const double w = ceil(sqrt((double)rb2[k]) * (1.0 + 1.0 / 1024.0) / h_grid[b]);
+            Bd.w[k] = (int8_t)(w < (double)P.w[k] ? w : (double)P.w[k]);
+        }
     uint32_t *parent = scratch, *min_id = scratch + P.n, *size = scratch + 2 * (size_t)P.n;
     uint32_t *root = B.val_in;            // free after the rebuild (arrival ranks / radix input values)
     k_cc_init<<<blocks_for(P.n), kThreads, 0, st>>>(P.n, parent, min_id, size);
