@@ -197,6 +197,31 @@ def test_hundred_steps(B, orc, name, n):
     sim.close()
 
 
+def test_full_size_trajectory_in_the_bench_configuration(B, orc):
+    """C3 at N = 2.5e5 exactly as bench.py times it (default kernels, tuned cells_per_cut,
+    CUDA-graph replay): one step to the one-step bars and 20 steps to 1e-3 R against the
+    oracle, every NP compared by id."""
+    w = workload("C3", None)
+    p = orc.params_from_workload(w)
+    sim = B.Simulation.from_workload(w, cells_per_cut=w.tuned_cells_per_cut)
+    x1o, v1o, bad = orc.step(p, w.pos, w.vel, w.type, step0=0, nsteps=1)
+    assert bad == 0
+    sim.step(1)
+    x, v, _, R, st = sim.get_state()
+    assert st == 1
+    assert np.abs(x.astype(np.float64) - x1o).max() <= 1e-5 * R
+    xo, vo, bad = orc.step(p, x1o, v1o, w.type, step0=1, nsteps=19)
+    assert bad == 0
+    sim.step(19)
+    x, v, _, R, st = sim.get_state()
+    assert st == 20
+    d = np.linalg.norm(x.astype(np.float64) - xo, axis=1)
+    assert d.max() <= 1e-3 * R, d.max() / R
+    m = np.asarray(w.mass)[w.type]
+    assert np.abs(v.astype(np.float64) - vo).max() <= 1e-2 * np.sqrt(w.kT / m.min())
+    sim.close()
+
+
 def test_noise_matches_oracle_draws(B, orc):
     """a = 0, no forces, v0 = 0  ->  v1 = b xi: the GPU's Philox/Box-Muller
     draws against the oracle's, particle by particle, at a 64-bit step index."""
