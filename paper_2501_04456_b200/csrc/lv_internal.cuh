@@ -106,7 +106,10 @@ __host__ __device__ inline double lv_radius_of(int mode, double R0, double R1, l
     return sqrt(R0 * R0 + (R1 * R1 - R0 * R0) * f);
 }
 
-constexpr int kScanTile = 4096;   // cells per tile of the cell-count scan
+#ifndef LV_SCAN_TILE
+#define LV_SCAN_TILE 8192
+#endif
+constexpr int kScanTile = LV_SCAN_TILE;   // cells per tile of the cell-count scan
 
 // ---- launch wrappers (lv_kernels.cu) -- all asynchronous on `st` ----------
 cudaError_t lvk_hash(const LvDev &P, const LvBufs &B, cudaStream_t st);

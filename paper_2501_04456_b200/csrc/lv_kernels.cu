@@ -154,8 +154,11 @@ k_hash_count(const __grid_constant__ LvDev P, const float4 *__restrict__ pos,
 // chained by decoupled look-back); cnt is zeroed behind the read so the next
 // step's histogram starts clean.  Look-back word = flag << 32 | value with
 // flag 1 = tile aggregate, 2 = inclusive prefix.
-constexpr int kScanThreads = 256;
-constexpr int kScanItems = kScanTile / kScanThreads;   // 16
+#ifndef LV_SCAN_ITEMS
+#define LV_SCAN_ITEMS 16
+#endif
+constexpr int kScanItems = LV_SCAN_ITEMS;
+constexpr int kScanThreads = kScanTile / kScanItems;
 
 __global__ void __launch_bounds__(kScanThreads)
 k_scan_cells(uint32_t n_items, uint32_t *__restrict__ cnt, uint32_t *__restrict__ off,
@@ -991,6 +994,8 @@ k_update(const __grid_constant__ LvDev P, const float4 *__restrict__ posB_,
     }
     const long long n = st->step;                      // index of this step
     const bool rebuilt = kList ? st->rebuild[n & 1] != 0u : true;
+    __shared__ double s_R;                             // (iii), R9: once per block, fp64
+    if (threadIdx.x == 0) s_R = lv_radius_of(P.sched_mode, P.R0, P.R1, P.sched_steps, n + 1);
     __syncthreads();
     // the block that takes the last ticket has seen every block read `step`
     if (threadIdx.x == 0 && atomicAdd(&st->ticket, 1u) == gridDim.x - 1) {
@@ -1001,7 +1006,7 @@ k_update(const __grid_constant__ LvDev P, const float4 *__restrict__ posB_,
     if (i >= P.n) return;
     const float4 *posB = rebuilt ? posB_ : posA;
     const float4 *velB = rebuilt ? velB_ : velA;
-    const double Rd = lv_radius_of(P.sched_mode, P.R0, P.R1, P.sched_steps, n + 1);  // (iii), R9
+    const double Rd = s_R;
     const float4 p = posB[i];
     const float4 v = velB[i];
     const float4 f = force[i];
