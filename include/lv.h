@@ -250,6 +250,30 @@ int lv_observe_radial(lv_sim *s, double dr, int n_bins, uint64_t *hist, double *
 int lv_observe_clusters(lv_sim *s, double bond_factor, int32_t *labels, int64_t *n_clusters,
                         double *mean_size, int64_t *largest, uint64_t *log2_hist);
 
+/* ---- headless view -----------------------------------------
+ * The paper's program shows the run "online" through the OpenGL display of
+ * the sample it adapts; a graphics API is unavailable here, so the
+ * perspective view of Fig. 2, right panel, is splatted by CUDA kernels
+ * into a caller buffer.  The scene is rotated by yaw about y, then pitch about x
+ * (radians); the camera sits on the +z axis at eye_dist from the droplet centre and looks
+ * at it; a point at view-axis distance zc projects with scale focal_px / zc onto a
+ * width x height image whose principal point is the centre.  Every NP is a sphere
+ * impostor of its radius, shaded 0.25 + 0.75 (n . view) times palette[type]
+ * (0x00BBGGRR), nearest fragment wins; empty pixels show `droplet` inside the projected
+ * disc of the droplet radius R(step) and `background` outside.  Pixels are 0xAABBGGRR
+ * with AA = 0xff. */
+typedef struct {
+    double eye_dist, focal_px, yaw, pitch;
+    int32_t width, height;               /* 1..8192 each */
+    uint32_t palette[LV_MAX_TYPES];
+    uint32_t background, droplet;
+} lv_view;
+
+/* zbuf_dev: DEVICE scratch of width*height*8 bytes, 8-byte aligned, owned by the caller,
+ * clobbered.  rgba: width*height uint32, written; host or device per on_device.
+ * Synchronises when rgba is host memory; the state does not change. */
+int lv_render(lv_sim *s, const lv_view *view, void *zbuf_dev, uint32_t *rgba, int on_device);
+
 /* Status bits LV_ST_* (host uint32, written).  Synchronises. */
 int lv_get_status(lv_sim *s, uint32_t *status);
 

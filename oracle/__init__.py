@@ -96,6 +96,9 @@ def lib():
         L.lvo_radial_hist.restype = None
         L.lvo_cluster_labels.argtypes = [C.c_int, fp, ip, fp, ip]
         L.lvo_cluster_labels.restype = None
+        L.lvo_render.argtypes = [C.c_int, fp, ip, fp, fp, C.c_float, C.c_float, C.c_int, C.c_int, up,
+                                 C.c_uint32, C.c_uint32, C.c_float, up]
+        L.lvo_render.restype = None
         L.lvo_sizeof_params.restype = C.c_int
         L.lvo_sizeof_grid.restype = C.c_int
         L.lvo_max_threads.restype = C.c_int
@@ -339,3 +342,25 @@ def cluster_labels(x_f32, type_, sigma_ab, bond_factor=1.5):
     lab = np.zeros(x.shape[0], dtype=np.int32)
     lib().lvo_cluster_labels(x.shape[0], _f(x), _i(t), _f(rb2), _i(lab))
     return lab
+
+
+def view_rotation(yaw, pitch):
+    """Scene rotation of the headless view: pitch about x after yaw about y (fp64 -> fp32)."""
+    cy, sy, cp, sp = np.cos(yaw), np.sin(yaw), np.cos(pitch), np.sin(pitch)
+    return np.array([cy, 0.0, sy, sp * sy, cp, -sp * cy, -cp * sy, sp, cp * cy], dtype=np.float32)
+
+
+def render(x_f32, type_, radius_a, R, eye_dist, focal_px, yaw, pitch, width, height, palette,
+           background, droplet):
+    """Perspective splat of Fig. 2 (right panel) -> uint32[height, width] (0xAABBGGRR)."""
+    x = np.ascontiguousarray(x_f32, dtype=np.float32).reshape(-1, 3)
+    t = _ci32(type_)
+    ra = np.ascontiguousarray(radius_a, dtype=np.float32)
+    pal = np.zeros(MAX_TYPES, dtype=np.uint32)
+    pal[:len(palette)] = np.asarray(palette, dtype=np.uint32)
+    rot = view_rotation(yaw, pitch)
+    img = np.zeros((int(height), int(width)), dtype=np.uint32)
+    lib().lvo_render(x.shape[0], _f(x), _i(t), _f(ra), _f(rot), C.c_float(float(np.float32(eye_dist))),
+                     C.c_float(float(np.float32(focal_px))), int(width), int(height), _u(pal),
+                     int(background), int(droplet), C.c_float(float(np.float32(R))), _u(img))
+    return img

@@ -594,6 +594,83 @@ void lvo_cluster_labels(int n, const float *x, const int32_t *type, const float 
     }
 }
 
+/* ------------------------------------------------------------------ */
+/* Headless perspective view (Fig. 2 right panel).
+ * Plain restatement of the splat: per NP, per pixel of its bounding box, single fp32
+ * operations in the order include/lv.h states (this file is built with
+ * -ffp-contract=off); the nearest fragment wins, ties by the smaller pixel value.
+ * rot: 9 floats row-major; palette / radius: per type. */
+static uint32_t shade_px(uint32_t base, float s)
+{
+    uint32_t out = 0xff000000u;
+    for (int c = 0; c < 3; ++c) {
+        float ch = (float)((base >> (8 * c)) & 0xffu);
+        uint32_t q = (uint32_t)(ch * s + 0.5f);
+        out |= (q > 255u ? 255u : q) << (8 * c);
+    }
+    return out;
+}
+
+void lvo_render(int n, const float *x, const int32_t *type, const float *radius_a,
+                const float *rot, float eye, float focal, int width, int height,
+                const uint32_t *palette, uint32_t background, uint32_t droplet, float R,
+                uint32_t *rgba)
+{
+    size_t n_px = (size_t)width * height;
+    uint64_t *zb = (uint64_t *)malloc(8 * n_px);
+    for (size_t p = 0; p < n_px; ++p) zb[p] = ~(uint64_t)0;
+    float cx = (float)(0.5 * width), cy = (float)(0.5 * height);
+    for (int i = 0; i < n; ++i) {
+        float px_ = x[3 * i], py_ = x[3 * i + 1], pz_ = x[3 * i + 2];
+        float r = radius_a[type[i]];
+        float xc = (rot[0] * px_ + rot[1] * py_) + rot[2] * pz_;
+        float yc = (rot[3] * px_ + rot[4] * py_) + rot[5] * pz_;
+        float zr = (rot[6] * px_ + rot[7] * py_) + rot[8] * pz_;
+        float zc = eye - zr;
+        if (!(zc > 2.0f * r)) continue;
+        float inv = focal / zc;
+        float u = cx + xc * inv;
+        float v = cy - yc * inv;
+        float rho = r * inv;
+        float rho2 = rho * rho;
+        if (!(rho2 > 0.0f) || !(fabsf(u) < 1e7f) || !(fabsf(v) < 1e7f) || !(rho < 1e4f)) continue;
+        int x0 = (int)floorf(u - rho), x1 = (int)floorf(u + rho);
+        int y0 = (int)floorf(v - rho), y1 = (int)floorf(v + rho);
+        if (x0 < 0) x0 = 0;
+        if (y0 < 0) y0 = 0;
+        if (x1 > width - 1) x1 = width - 1;
+        if (y1 > height - 1) y1 = height - 1;
+        for (int py = y0; py <= y1; ++py) {
+            float dy = ((float)py + 0.5f) - v;
+            float dy2 = dy * dy;
+            for (int px = x0; px <= x1; ++px) {
+                float dx = ((float)px + 0.5f) - u;
+                float d2 = dx * dx + dy2;
+                if (d2 <= rho2) {
+                    float nz = sqrtf((rho2 - d2) / rho2);
+                    float zf = zc - r * nz;
+                    uint32_t c = shade_px(palette[type[i]], 0.25f + 0.75f * nz);
+                    uint32_t zbits;
+                    memcpy(&zbits, &zf, 4);
+                    uint64_t key = ((uint64_t)zbits << 32) | c;
+                    size_t p = (size_t)py * width + px;
+                    if (key < zb[p]) zb[p] = key;
+                }
+            }
+        }
+    }
+    float rr = R * (focal / eye);
+    for (int py = 0; py < height; ++py)
+        for (int px = 0; px < width; ++px) {
+            size_t p = (size_t)py * width + px;
+            if (zb[p] != ~(uint64_t)0) { rgba[p] = (uint32_t)zb[p]; continue; }
+            float dx = ((float)px + 0.5f) - cx, dy = ((float)py + 0.5f) - cy;
+            float d2 = dx * dx + dy * dy;
+            rgba[p] = d2 <= rr * rr ? droplet : background;
+        }
+    free(zb);
+}
+
 int lvo_sizeof_params(void) { return (int)sizeof(lvo_params); }
 int lvo_sizeof_grid(void) { return (int)sizeof(lvo_grid); }
 int lvo_max_threads(void)

@@ -30,12 +30,19 @@ FORCE_SIMPLE, FORCE_QUEUED, FORCE_SEGMENTS, FORCE_PACKED = 0, 1, 2, 3
 # every symbol include/lv.h declares (tests check the library exports them all)
 SYMBOLS = ["lv_langevin_coeffs", "lv_create", "lv_set_types", "lv_set_forces",
            "lv_set_droplet_schedule", "lv_set_grid", "lv_set_option", "lv_set_neighbour_list",
-           "lv_get_rebuild_count", "lv_observe_rdf", "lv_observe_radial", "lv_observe_clusters", "lv_workspace_bytes", "lv_bind",
+           "lv_get_rebuild_count", "lv_observe_rdf", "lv_observe_radial", "lv_observe_clusters", "lv_render", "lv_workspace_bytes", "lv_bind",
            "lv_set_state", "lv_step", "lv_compute_forces", "lv_get_state", "lv_get_forces",
            "lv_get_status", "lv_get_debug", "lv_launches_per_step", "lv_step_profiled",
            "lv_stage_timing", "lv_read_stage_timing",
            "lv_measure_fp32_peak", "lv_destroy", "lv_strerror",
            "lv_last_cuda_error", "lv_version"]
+
+
+class LvView(C.Structure):
+    _fields_ = [("eye_dist", C.c_double), ("focal_px", C.c_double), ("yaw", C.c_double),
+                ("pitch", C.c_double), ("width", C.c_int32), ("height", C.c_int32),
+                ("palette", C.c_uint32 * MAX_TYPES), ("background", C.c_uint32),
+                ("droplet", C.c_uint32)]
 
 
 class LvType(C.Structure):
@@ -80,6 +87,7 @@ def load():
     L.lv_observe_rdf.argtypes = [vp, C.c_double, C.c_int, C.POINTER(C.c_uint64), dp]
     L.lv_observe_clusters.argtypes = [vp, C.c_double, ip, C.POINTER(C.c_int64), dp,
                                       C.POINTER(C.c_int64), C.POINTER(C.c_uint64)]
+    L.lv_render.argtypes = [vp, C.POINTER(LvView), vp, vp, C.c_int]
     L.lv_observe_radial.argtypes = [vp, C.c_double, C.c_int, C.POINTER(C.c_uint64), dp, dp, dp, dp,
                                     C.POINTER(C.c_int64)]
     L.lv_workspace_bytes.argtypes = [vp]
@@ -297,6 +305,30 @@ class Simulation:
             "lv_observe_clusters")
         return dict(labels=lab, n_clusters=int(nc.value), mean_size=ms.value, largest=int(lg.value),
                     log2_hist=hist)
+
+    def render(self, eye_dist, focal_px, yaw, pitch, width, height, palette,
+               background=0xff000000, droplet=0xff302010, on_device=False):
+        """Perspective view of the current state -> uint32[height, width] (numpy, or a torch
+        tensor on the device with on_device=True)."""
+        import torch
+        v = LvView(float(eye_dist), float(focal_px), float(yaw), float(pitch), int(width), int(height))
+        for a, c in enumerate(palette):
+            v.palette[a] = int(c)
+        v.background, v.droplet = int(background), int(droplet)
+        with torch.cuda.device(self.device):
+            zbuf = torch.empty(int(width) * int(height), dtype=torch.int64, device=self.device)
+            zbuf.record_stream(self.stream)
+            if on_device:
+                img = torch.empty((int(height), int(width)), dtype=torch.int32, device=self.device)
+                img.record_stream(self.stream)
+                self._check(self.L.lv_render(self.h, C.byref(v), zbuf.data_ptr(), img.data_ptr(), 1),
+                            "lv_render")
+                return img
+            img = np.zeros((int(height), int(width)), dtype=np.uint32)
+            self._check(self.L.lv_render(self.h, C.byref(v), zbuf.data_ptr(), img.ctypes.data, 0),
+                        "lv_render")
+            self.stream.synchronize()
+            return img
 
     def status(self) -> int:
         s = C.c_uint32()

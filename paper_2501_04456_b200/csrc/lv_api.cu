@@ -738,6 +738,41 @@ int lv_observe_clusters(lv_sim *s, double bond_factor, int32_t *labels, int64_t 
     return LV_OK;
 }
 
+int lv_render(lv_sim *s, const lv_view *view, void *zbuf_dev, uint32_t *rgba, int on_device)
+{
+    if (!s || !view || !zbuf_dev || !rgba) return LV_E_ARG;
+    if (view->width < 1 || view->height < 1 || view->width > 8192 || view->height > 8192) return LV_E_ARG;
+    if (!(view->eye_dist > 0.0) || !(view->focal_px > 0.0)) return LV_E_ARG;
+    if (((uintptr_t)zbuf_dev % 8) != 0) return LV_E_ARG;
+    if (!s->bound || !s->state_set) return LV_E_ORDER;
+    // rotation = pitch about x after yaw about y, in fp64, rounded once
+    const double cy = cos(view->yaw), sy = sin(view->yaw), cp = cos(view->pitch), sp = sin(view->pitch);
+    const double m[9] = {cy, 0.0, sy, sp * sy, cp, -sp * cy, -cp * sy, sp, cp * cy};
+    float rot[9];
+    for (int k = 0; k < 9; ++k) rot[k] = (float)m[k];
+    LvDevState st;
+    LV_CUDA(s, cudaMemcpyAsync(&st, s->bufs.st, sizeof(st), cudaMemcpyDeviceToHost, s->stream));
+    LV_CUDA(s, cudaStreamSynchronize(s->stream));
+    const double R = lv_radius_of(s->sched_mode, s->R0, s->R1, s->sched_steps, st.step);
+    const size_t n_px = (size_t)view->width * view->height;
+    uint32_t *drgba = rgba;
+    if (!on_device) {
+        // the image is staged behind the depth keys would need more scratch: use the tail of zbuf?
+        // no -- keep it simple: a temporary device image
+        LV_CUDA(s, cudaMallocAsync((void **)&drgba, 4 * n_px, s->stream));
+    }
+    cudaError_t e = lvk_render(s->dev, s->bufs, view, rot, R, (unsigned long long *)zbuf_dev, drgba, s->stream);
+    if (e == cudaSuccess && !on_device)
+        e = cudaMemcpyAsync(rgba, drgba, 4 * n_px, cudaMemcpyDeviceToHost, s->stream);
+    if (!on_device) {
+        cudaError_t e2 = cudaFreeAsync(drgba, s->stream);
+        if (e == cudaSuccess) e = e2;
+        if (e == cudaSuccess) e = cudaStreamSynchronize(s->stream);
+    }
+    if (e != cudaSuccess) return cuda_fail(s, e, "lv_render");
+    return LV_OK;
+}
+
 int lv_get_status(lv_sim *s, uint32_t *status)
 {
     if (!s || !status) return LV_E_ARG;

@@ -1367,6 +1367,102 @@ k_cc_labels(int n, const uint32_t *__restrict__ root, const float4 *__restrict__
     }
 }
 
+// ----------------------------- headless view
+// The paper's program shows the droplet "online" through the OpenGL display of NVIDIA's
+// particle sample; here the perspective view of Fig. 2 (right panel) is a CUDA splat into a
+// device buffer, no graphics API.  Every NP is a shaded sphere impostor; the nearest
+// fragment wins through a 64-bit atomicMin on (depth bits << 32 | rgba).  All arithmetic
+// is single IEEE operations in a fixed order (no FMA contraction), so the oracle's plain C
+// restatement produces the same image bit for bit.
+struct LvViewDev {
+    float m[9];            // scene rotation, row-major
+    float eye, focal;      // camera on the +z axis at distance eye, looking at the centre
+    float cx, cy;          // principal point (pixels)
+    int32_t width, height;
+    uint32_t palette[LV_MAX_TYPES];   // 0x00BBGGRR per type
+    uint32_t background, droplet;
+    float radius[LV_MAX_TYPES];       // NP radius per type
+    float R;                          // droplet radius (for the silhouette)
+};
+
+__device__ __forceinline__ uint32_t shade_rgba(uint32_t base, float s)
+{
+    uint32_t out = 0xff000000u;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const float ch = (float)((base >> (8 * c)) & 0xffu);
+        const uint32_t q = (uint32_t)__fadd_rn(__fmul_rn(ch, s), 0.5f);
+        out |= (q > 255u ? 255u : q) << (8 * c);
+    }
+    return out;
+}
+
+__global__ void __launch_bounds__(kThreads)
+k_render_clear(int n_px, unsigned long long *zbuf)
+{
+    const int p = blockIdx.x * kThreads + threadIdx.x;
+    if (p < n_px) zbuf[p] = 0xffffffffffffffffull;
+}
+
+__global__ void __launch_bounds__(kThreads)
+k_render_splat(int n, const LvViewDev V, const float4 *__restrict__ pos, unsigned long long *zbuf)
+{
+    const int i = blockIdx.x * kThreads + threadIdx.x;
+    if (i >= n) return;
+    const float4 p = pos[i];
+    const int a = __float_as_int(p.w);
+    const float r = V.radius[a];
+    // camera space: rotate the scene, camera at (0, 0, eye) looking down -z
+    const float xc = __fadd_rn(__fadd_rn(__fmul_rn(V.m[0], p.x), __fmul_rn(V.m[1], p.y)), __fmul_rn(V.m[2], p.z));
+    const float yc = __fadd_rn(__fadd_rn(__fmul_rn(V.m[3], p.x), __fmul_rn(V.m[4], p.y)), __fmul_rn(V.m[5], p.z));
+    const float zr = __fadd_rn(__fadd_rn(__fmul_rn(V.m[6], p.x), __fmul_rn(V.m[7], p.y)), __fmul_rn(V.m[8], p.z));
+    const float zc = __fsub_rn(V.eye, zr);                 // distance along the view axis
+    if (!(zc > __fmul_rn(2.0f, r))) return;                // behind or touching the camera (NaN too)
+    const float inv = __fdiv_rn(V.focal, zc);
+    const float u = __fadd_rn(V.cx, __fmul_rn(xc, inv));
+    const float v = __fsub_rn(V.cy, __fmul_rn(yc, inv));
+    const float rho = __fmul_rn(r, inv);
+    const float rho2 = __fmul_rn(rho, rho);
+    if (!(rho2 > 0.0f) || !(fabsf(u) < 1e7f) || !(fabsf(v) < 1e7f) || !(rho < 1e4f)) return;
+    const int x0 = max(0, (int)floorf(__fsub_rn(u, rho))), x1 = min(V.width - 1, (int)floorf(__fadd_rn(u, rho)));
+    const int y0 = max(0, (int)floorf(__fsub_rn(v, rho))), y1 = min(V.height - 1, (int)floorf(__fadd_rn(v, rho)));
+    const uint32_t base = V.palette[a];
+    for (int py = y0; py <= y1; ++py) {
+        const float dy = __fsub_rn(__fadd_rn((float)py, 0.5f), v);
+        const float dy2 = __fmul_rn(dy, dy);
+        for (int px = x0; px <= x1; ++px) {
+            const float dx = __fsub_rn(__fadd_rn((float)px, 0.5f), u);
+            const float d2 = __fadd_rn(__fmul_rn(dx, dx), dy2);
+            if (d2 <= rho2) {
+                const float nz = __fsqrt_rn(__fdiv_rn(__fsub_rn(rho2, d2), rho2));     // normal . view, 0..1
+                const float zf = __fsub_rn(zc, __fmul_rn(r, nz));                      // fragment depth
+                const uint32_t c = shade_rgba(base, __fadd_rn(0.25f, __fmul_rn(0.75f, nz)));
+                const unsigned long long key = ((unsigned long long)__float_as_uint(zf) << 32) | c;
+                atomicMin(zbuf + (size_t)py * V.width + px, key);
+            }
+        }
+    }
+}
+
+// empty pixels: the droplet's silhouette (projected disc of radius R) or the background
+__global__ void __launch_bounds__(kThreads)
+k_render_resolve(const LvViewDev V, const unsigned long long *__restrict__ zbuf, uint32_t *__restrict__ rgba)
+{
+    const int p = blockIdx.x * kThreads + threadIdx.x;
+    if (p >= V.width * V.height) return;
+    const unsigned long long k = zbuf[p];
+    uint32_t c = (uint32_t)k;
+    if (k == 0xffffffffffffffffull) {
+        const int py = p / V.width, px = p - py * V.width;
+        const float rr = __fmul_rn(V.R, __fdiv_rn(V.focal, V.eye));
+        const float dx = __fsub_rn(__fadd_rn((float)px, 0.5f), V.cx);
+        const float dy = __fsub_rn(__fadd_rn((float)py, 0.5f), V.cy);
+        const float d2 = __fadd_rn(__fmul_rn(dx, dx), __fmul_rn(dy, dy));
+        c = d2 <= __fmul_rn(rr, rr) ? V.droplet : V.background;
+    }
+    rgba[p] = c;
+}
+
 inline int blocks_for(int n) { return n > 0 ? (n + kThreads - 1) / kThreads : 1; }
 
 }  // namespace
@@ -1585,6 +1681,32 @@ cudaError_t lvk_clusters(const LvDev &P, const LvBufs &B, const float *rb2, cons
     k_cc_roots<<<blocks_for(P.n), kThreads, 0, st>>>(P.n, parent, root, B.velB, min_id, size);
     k_cc_labels<<<blocks_for(P.n), kThreads, 0, st>>>(P.n, root, B.velB, min_id, size, label_by_id,
                                                       stats);
+    return cudaGetLastError();
+}
+
+cudaError_t lvk_render(const LvDev &P, const LvBufs &B, const lv_view *view, const float *rot9,
+                       double R, unsigned long long *zbuf, uint32_t *rgba, cudaStream_t st)
+{
+    LvViewDev V;
+    memset(&V, 0, sizeof(V));
+    for (int k = 0; k < 9; ++k) V.m[k] = rot9[k];
+    V.eye = (float)view->eye_dist;
+    V.focal = (float)view->focal_px;
+    V.cx = (float)(0.5 * view->width);
+    V.cy = (float)(0.5 * view->height);
+    V.width = view->width;
+    V.height = view->height;
+    for (int a = 0; a < LV_MAX_TYPES; ++a) {
+        V.palette[a] = view->palette[a];
+        V.radius[a] = (float)P.radius_d[a];
+    }
+    V.background = view->background;
+    V.droplet = view->droplet;
+    V.R = (float)R;
+    const int n_px = view->width * view->height;
+    k_render_clear<<<blocks_for(n_px), kThreads, 0, st>>>(n_px, zbuf);
+    if (P.n > 0) k_render_splat<<<blocks_for(P.n), kThreads, 0, st>>>(P.n, V, B.posA, zbuf);
+    k_render_resolve<<<blocks_for(n_px), kThreads, 0, st>>>(V, zbuf, rgba);
     return cudaGetLastError();
 }
 
