@@ -277,7 +277,18 @@ def run_lv(args):
         for _ in range(5):
             cl = sim.observe_clusters(1.5, want_labels=False)
         t_cl = (time.perf_counter() - t0) / 5
+        pal = [0x00ff8040, 0x004080ff, 0x0040ff80, 0x00c0c0c0]
+        eye = 2.6 * w.R0
+        sim.render(eye, 900.0 * eye / (2.2 * w.R0), 0.4, 0.3, 1920, 1080, pal, on_device=True)
+        sim.synchronize()
+        t0 = time.perf_counter()
+        for _ in range(5):
+            sim.render(eye, 900.0 * eye / (2.2 * w.R0), 0.4, 0.3, 1920, 1080, pal, on_device=True)
+        sim.synchronize()
+        t_view = (time.perf_counter() - t0) / 5
         observables = {
+            "view": {"ms": t_view * 1e3, "width": 1920, "height": 1080,
+                     "how": "lv_render: 1920x1080 perspective splat of all NPs into a device buffer, wall clock"},
             "clusters": {"ms": t_cl * 1e3, "bond_factor": 1.5, "n_clusters": cl["n_clusters"],
                          "largest": cl["largest"],
                          "how": "lv_observe_clusters: cell rebuild + union-find + statistics, wall clock"},
