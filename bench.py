@@ -336,7 +336,16 @@ def run_lv(args):
         "kernel": "k_pair_force_s" if args.force_kernel in (None, 2, 3) else "k_pair_force", "bound": "alu",
         "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s",
         "frac": achieved / peak_tflops,
-        "traffic": args.force_traffic_bytes,
+        # dram__bytes_read.sum + dram__bytes_write.sum of k_pair_force_s per launch from the committed
+        # ncu --set full capture of this command (profiles/r1c_segments_C3.md: 6.90 MB read, 0 written);
+        # only meaningful for the default kernel and workload it was captured on
+        "traffic": args.force_traffic_bytes if args.force_traffic_bytes is not None else (
+            6.8965e6 if (w.name == "C3" and args.force_kernel in (None, 2) and args.start_step == 0
+                         and nl is None) else None),
+        "traffic_source": "profiles/r1c_segments_C3.md (ncu --set full, cold cache); algorithmic 32 B/NP = "
+                          f"{32 * n} B",
+        "executed_fp32_util_ncu": "21 % of FP32-lane slots at step 0, 31 % at step 17 000 "
+                                  "(profiles/r1c_segments_C3.md, r1d_dense_states_C3.md)",
         "peak_source": f"{n_sms} SMs x 128 FP32 lanes x 2 x {pk['sm_max_mhz']:.0f} MHz "
                        f"(DESIGN.md); measured FMA microkernel {fma_tflops:.1f} TFLOP/s",
         "algorithmic_flops_per_launch": flops,
