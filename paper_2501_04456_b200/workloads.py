@@ -120,6 +120,35 @@ def _spec(name: str) -> Workload:
                         wall_mode=WALL_ONESIDED, sched_mode=SCHED_LINEAR, R0=250.0, R1=120.0,
                         sched_steps=10000, seed=5, steps=10000, init="ball", tuned_cells_per_cut=[1, 1],
                         tuned_neighbour_list=(0.4, 128))
+    # ---- paper-shaped scenarios (Table 1) in reduced units; synthetic
+    # stand-ins: the authors' parameter files are not available
+    if name == "P1":
+        # row "1" (Fig. 2, 7): R0 = 20 um, r_NP = 0.5 um -> sigma = 1, R0 = 20; 10^4 neutral NPs,
+        # LJ only, range 4 (r_A + r_B), no evaporation, random tumbling =
+        # isotropic centrifugal force; the paper's windowed surface force
+        s = [1.0]
+        w2 = 0.05 ** 2
+        return Workload("P1", 10000, s, [1.0], [0.0], _mass(s), [100.0], [1.0], [1.0],
+                        kT=1.0, dt=0.005, cut_factor=4.0, coulomb_k=0.0, g=0.0,
+                        omega2=(w2, w2, w2), wall_mode=WALL_WINDOW,
+                        sched_mode=SCHED_CONST, R0=20.0, R1=20.0, sched_steps=0,
+                        seed=11, steps=5000, init="ball", tuned_cells_per_cut=[2],
+                        tuned_neighbour_list=(0.3, 256))
+    if name == "P8":
+        # row "8" (Fig. 8, 9): R0 = 60 um, r_NP = 0.25 / 1.5 um (6 : 1) -> sigma = 1 / 6,
+        # R0 = 120; 39 500 + 1 500 neutral NPs; eps = 0.23 [[0.155, 0.155], [0, 1.26]] is not a
+        # Berthelot matrix (and prints a 0 below the diagonal: read as symmetric), here in units
+        # of eps_11; radius-square-law evaporation until nearly dry; rotation
+        # about one axis
+        s = [1.0, 6.0]
+        w2 = 0.01 ** 2
+        eps = np.array([[1.0, 1.0], [1.0, 1.26 / 0.155]])
+        return Workload("P8", 41000, s, [1.0, 1.26 / 0.155], [0.0, 0.0], _mass(s), [100.0] * 2,
+                        [1.0] * 2, [39500.0 / 41000.0, 1500.0 / 41000.0], kT=1.0, dt=0.002,
+                        cut_factor=4.0, coulomb_k=0.0, g=0.0, omega2=(w2, w2, 0.0),
+                        wall_mode=WALL_ONESIDED, sched_mode=SCHED_R2LAW, R0=120.0, R1=48.0,
+                        sched_steps=20000, seed=18, steps=20000, init="ball", eps_matrix=eps,
+                        tuned_cells_per_cut=[1, 3], tuned_neighbour_list=(0.4, 512))
     raise KeyError(name)
 
 
@@ -210,7 +239,7 @@ def fcc_ball(rng, n, sigma, R, jitter=0.05):
 
 def make_workload(name: str, n: Optional[int] = None, state: bool = True,
                   seed: Optional[int] = None) -> Workload:
-    """BASELINE config `name` ("C1".."C5").  With n given, a scaled-down (or
+    """BASELINE config `name` ("C1".."C5") or paper-shaped scenario ("P1", "P8").  With n given, a scaled-down (or
     up) copy at the same volume fractions: radii scale as (n/N)^(1/3).  `seed`
     overrides the configuration's seed (independent replicas)."""
     w = _spec(name)

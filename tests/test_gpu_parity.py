@@ -222,6 +222,40 @@ def test_full_size_trajectory_in_the_bench_configuration(B, orc):
     sim.close()
 
 
+@pytest.mark.parametrize("name", ["P1", "P8"])
+def test_paper_shaped_scenarios(B, orc, name):
+    """Table 1 shapes at full size: P1 = 10^4 NPs, range 4 sigma, isotropic
+    centrifugal force, windowed wall; P8 = 39 500 + 1 500 NPs with a 6 : 1 size ratio, the
+    non-Berthelot eps matrix and radius-square-law evaporation.  Cell structures and counts
+    bit-exact, forces to 1e-5, 100 steps to 1e-3 R, with and without the neighbour list."""
+    w = workload(name, None)
+    p = orc.params_from_workload(w)
+    cpc = w.tuned_cells_per_cut
+    g = orc.grid_spec(p, cpc)
+    key, ks, perm, off = orc.cell_structures(g, w.pos, w.type)
+    Fo, So, co, _ = orc.pair_forces(p, w.pos, w.type, "cells")
+    sim = B.Simulation.from_workload(w, cells_per_cut=cpc)
+    sim.compute_forces()
+    assert np.array_equal(sim.get_debug(B.DBG_KEYS_SORTED), ks)
+    assert np.array_equal(sim.get_debug(B.DBG_PERM), perm)
+    assert np.array_equal(sim.get_debug(B.DBG_CELL_OFFSETS), off)
+    Fg, cg = sim.get_forces()
+    assert np.array_equal(cg, co) and co.sum() > 0
+    assert force_error(Fg, Fo, So) <= FORCE_TOL
+    xo, vo, bad = orc.step(p, w.pos, w.vel, w.type, step0=0, nsteps=100)
+    assert bad == 0
+    sim.step(100)
+    x, v, _, R, st = sim.get_state()
+    assert st == 100 and R == pytest.approx(orc.radius(p, 100), rel=1e-15)
+    assert np.linalg.norm(x.astype(np.float64) - xo, axis=1).max() <= 1e-3 * R
+    lst = B.Simulation.from_workload(w, cells_per_cut=cpc, neighbour_list=w.tuned_neighbour_list)
+    lst.step(100)
+    xl, vl, _, _, _ = lst.get_state()
+    assert np.linalg.norm(xl.astype(np.float64) - xo, axis=1).max() <= 1e-3 * R
+    assert 1 <= lst.rebuild_count() < 100
+    sim.close(); lst.close()
+
+
 def test_noise_matches_oracle_draws(B, orc):
     """a = 0, no forces, v0 = 0  ->  v1 = b xi: the GPU's Philox/Box-Muller
     draws against the oracle's, particle by particle, at a 64-bit step index."""
