@@ -259,6 +259,34 @@ def run_lv(args):
         }
         vs.close()
 
+    # ---- variant: many small droplets at once (NEXT-3 batched replicas; the paper's own
+    # sizes, Table 1: 10^4 NPs, fill a fraction of a B200) -- R handles on R streams
+    if rank == 0 and world == 1 and not args.no_variants and args.small_replicas > 0:
+        ks = 1000
+        sr = {}
+        for R_ in (1, args.small_replicas):
+            rs = replicas.ReplicaSet(lambda seed: workloads.make_workload("P1", seed=seed), R_,
+                                     base_seed=1234, device=device)
+            rs.step(100)
+            rs.synchronize()
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            rs.step(ks)
+            rs.synchronize()
+            dt_ = time.perf_counter() - t0
+            sr[R_] = {"ms_per_step_of_all": dt_ / ks * 1e3,
+                      "value": rs.n_particles * ks / dt_, "unit": UNIT}
+            npart = rs.workloads[0].n
+            rs.close()
+        variants["small_replicas"] = {
+            "what": "replicas.ReplicaSet: independent P1 droplets (Table 1 row 1 shape, N = %d each) "
+                    "stepped concurrently on one GPU, one lv_sim handle and stream per replica; "
+                    "each replica bit-identical to its solo run (test_replica_set_equals_solo_runs); "
+                    "wall clock over %d resident steps, no L2 flush" % (npart, ks),
+            "replicas": {str(k): v for k, v in sr.items()},
+            "speedup": sr[args.small_replicas]["value"] / sr[1]["value"],
+        }
+
     # ---- NEXT-1 rows: the paper's observables on the device (synchronous calls) -------
     observables = {}
     if rank == 0 and world == 1 and not args.no_variants:
@@ -494,6 +522,8 @@ def main():
     ap.add_argument("--neighbour-list", type=float, nargs=2, default=None, metavar=("SKIN", "CAP"),
                     help="lv_set_neighbour_list: time the skin-list variant instead of the per-step rebuild")
     ap.add_argument("--no-variants", action="store_true", help="skip the skin-list variant")
+    ap.add_argument("--small-replicas", type=int, default=16,
+                    help="size of the concurrent small-droplet replica set of the variants leg (0: skip)")
     ap.add_argument("--e2e-steps", type=int, default=0)
     ap.add_argument("--snapshots", type=int, nargs="*", default=[10000, 17000])
     ap.add_argument("--snapshot-steps", type=int, default=100)

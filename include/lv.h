@@ -274,6 +274,33 @@ typedef struct {
  * Synchronises when rgba is host memory; the state does not change. */
 int lv_render(lv_sim *s, const lv_view *view, void *zbuf_dev, uint32_t *rgba, int on_device);
 
+/* lv_render_surface: the LEFT panel of Fig. 2, "projection of the microdroplet surface onto
+ * a plane", where "circles/ellipses (circles elongated due to the projection) correspond to
+ * the NPs intersections with the microdroplet surface".  The paper does
+ * not name the projection; this build takes the equirectangular map (longitude x latitude,
+ * pole = z axis), which elongates circles along the longitude towards the poles as the
+ * caption describes.  Pixel (px, py) of a width x height image looks at
+ *   lambda = -pi + 2 pi (px + 0.5) / width,   phi = pi/2 - pi (py + 0.5) / height,
+ * its direction is d = (cos phi cos lambda, cos phi sin lambda, sin phi) with the four
+ * factors evaluated in fp64 and rounded once to fp32, and its surface point is
+ * s = (R cl_phi c_lambda, R cl_phi s_lambda, R s_phi) -- fp32, products left to right as
+ * written: R * (cos phi * cos lambda) etc. -- with R = fl32(R(step)).  NP i marks the pixel
+ * iff d2 = ((sx-x)^2 + (sy-y)^2) + (sz-z)^2 < r_a * r_a (single fp32 operations, no FMA, r_a the
+ * fp32 NP radius);
+ * among several the smallest (bits(d2) << 32 | palette[type]) wins; a pixel no NP marks
+ * shows `droplet`.  Pixels are 0xAABBGGRR with AA = 0xff.
+ * scratch_dev: DEVICE scratch of width*height*8 + (width + height)*8 bytes, 8-byte aligned,
+ * owned by the caller, clobbered.  rgba: width*height uint32, host or device per on_device.
+ * Synchronises; the state does not change. */
+typedef struct {
+    int32_t width, height;               /* 1..8192 each */
+    uint32_t palette[LV_MAX_TYPES];      /* 0x00BBGGRR per type */
+    uint32_t droplet;
+} lv_surface_map;
+
+int lv_render_surface(lv_sim *s, const lv_surface_map *map, void *scratch_dev, uint32_t *rgba,
+                      int on_device);
+
 /* Status bits LV_ST_* (host uint32, written).  Synchronises. */
 int lv_get_status(lv_sim *s, uint32_t *status);
 

@@ -99,6 +99,9 @@ def lib():
         L.lvo_render.argtypes = [C.c_int, fp, ip, fp, fp, C.c_float, C.c_float, C.c_int, C.c_int, up,
                                  C.c_uint32, C.c_uint32, C.c_float, up]
         L.lvo_render.restype = None
+        L.lvo_render_surface.argtypes = [C.c_int, fp, ip, fp, C.c_float, C.c_int, C.c_int, up,
+                                         C.c_uint32, up]
+        L.lvo_render_surface.restype = None
         L.lvo_sizeof_params.restype = C.c_int
         L.lvo_sizeof_grid.restype = C.c_int
         L.lvo_max_threads.restype = C.c_int
@@ -363,4 +366,18 @@ def render(x_f32, type_, radius_a, R, eye_dist, focal_px, yaw, pitch, width, hei
     lib().lvo_render(x.shape[0], _f(x), _i(t), _f(ra), _f(rot), C.c_float(float(np.float32(eye_dist))),
                      C.c_float(float(np.float32(focal_px))), int(width), int(height), _u(pal),
                      int(background), int(droplet), C.c_float(float(np.float32(R))), _u(img))
+    return img
+
+
+def render_surface(x_f32, type_, radius_a, R, width, height, palette, droplet):
+    """Equirectangular map of the NP intersections with the droplet surface, Fig. 2 left panel
+    (projection: this build's reading, include/lv.h) -> uint32[height, width]."""
+    x = np.ascontiguousarray(x_f32, dtype=np.float32).reshape(-1, 3)
+    t = _ci32(type_)
+    ra = np.ascontiguousarray(radius_a, dtype=np.float32)
+    pal = np.zeros(MAX_TYPES, dtype=np.uint32)
+    pal[:len(palette)] = np.asarray(palette, dtype=np.uint32)
+    img = np.zeros((int(height), int(width)), dtype=np.uint32)
+    lib().lvo_render_surface(x.shape[0], _f(x), _i(t), _f(ra), C.c_float(float(np.float32(R))),
+                             int(width), int(height), _u(pal), int(droplet), _u(img))
     return img

@@ -671,6 +671,43 @@ void lvo_render(int n, const float *x, const int32_t *type, const float *radius_
     free(zb);
 }
 
+/* Surface map, the left panel of Fig. 2 ("projection of the microdroplet
+ * surface onto a plane", NP intersections with the surface as circles "elongated due to the
+ * projection"); the projection is this build's reading (equirectangular, pole = z), its
+ * definition is in include/lv.h.  Written as the definition: for EVERY pixel, the surface
+ * point it looks at, then EVERY NP tested against it -- no windows, no culling.  The
+ * direction factors are fp64 libm values rounded once to fp32; the coverage test is single
+ * fp32 operations in the stated order (-ffp-contract=off). */
+void lvo_render_surface(int n, const float *x, const int32_t *type, const float *radius_a,
+                        float R, int width, int height, const uint32_t *palette,
+                        uint32_t droplet, uint32_t *rgba)
+{
+    const double pi = 3.14159265358979323846;
+#pragma omp parallel for schedule(static)
+    for (int py = 0; py < height; ++py) {
+        double phi = 0.5 * pi - pi * (((double)py + 0.5) / (double)height);
+        float cl = (float)cos(phi), sl = (float)sin(phi);
+        for (int px = 0; px < width; ++px) {
+            double lam = -pi + (2.0 * pi) * (((double)px + 0.5) / (double)width);
+            float co = (float)cos(lam), so = (float)sin(lam);
+            float sx = R * (cl * co), sy = R * (cl * so), sz = R * sl;
+            uint64_t best = ~(uint64_t)0;
+            for (int i = 0; i < n; ++i) {
+                float r = radius_a[type[i]];
+                float dx = sx - x[3 * i], dy = sy - x[3 * i + 1], dz = sz - x[3 * i + 2];
+                float d2 = (dx * dx + dy * dy) + dz * dz;
+                if (d2 < r * r) {
+                    uint32_t bits;
+                    memcpy(&bits, &d2, 4);
+                    uint64_t key = ((uint64_t)bits << 32) | (palette[type[i]] | 0xff000000u);
+                    if (key < best) best = key;
+                }
+            }
+            rgba[(size_t)py * width + px] = best == ~(uint64_t)0 ? droplet : (uint32_t)best;
+        }
+    }
+}
+
 int lvo_sizeof_params(void) { return (int)sizeof(lvo_params); }
 int lvo_sizeof_grid(void) { return (int)sizeof(lvo_grid); }
 int lvo_max_threads(void)

@@ -30,7 +30,7 @@ FORCE_SIMPLE, FORCE_QUEUED, FORCE_SEGMENTS, FORCE_PACKED = 0, 1, 2, 3
 # every symbol include/lv.h declares (tests check the library exports them all)
 SYMBOLS = ["lv_langevin_coeffs", "lv_create", "lv_set_types", "lv_set_forces",
            "lv_set_droplet_schedule", "lv_set_grid", "lv_set_option", "lv_set_neighbour_list",
-           "lv_get_rebuild_count", "lv_observe_rdf", "lv_observe_radial", "lv_observe_clusters", "lv_render", "lv_workspace_bytes", "lv_bind",
+           "lv_get_rebuild_count", "lv_observe_rdf", "lv_observe_radial", "lv_observe_clusters", "lv_render", "lv_render_surface", "lv_workspace_bytes", "lv_bind",
            "lv_set_state", "lv_step", "lv_compute_forces", "lv_get_state", "lv_get_forces",
            "lv_get_status", "lv_get_debug", "lv_launches_per_step", "lv_step_profiled",
            "lv_stage_timing", "lv_read_stage_timing",
@@ -43,6 +43,11 @@ class LvView(C.Structure):
                 ("pitch", C.c_double), ("width", C.c_int32), ("height", C.c_int32),
                 ("palette", C.c_uint32 * MAX_TYPES), ("background", C.c_uint32),
                 ("droplet", C.c_uint32)]
+
+
+class LvSurfaceMap(C.Structure):
+    _fields_ = [("width", C.c_int32), ("height", C.c_int32),
+                ("palette", C.c_uint32 * MAX_TYPES), ("droplet", C.c_uint32)]
 
 
 class LvType(C.Structure):
@@ -88,6 +93,7 @@ def load():
     L.lv_observe_clusters.argtypes = [vp, C.c_double, ip, C.POINTER(C.c_int64), dp,
                                       C.POINTER(C.c_int64), C.POINTER(C.c_uint64)]
     L.lv_render.argtypes = [vp, C.POINTER(LvView), vp, vp, C.c_int]
+    L.lv_render_surface.argtypes = [vp, C.POINTER(LvSurfaceMap), vp, vp, C.c_int]
     L.lv_observe_radial.argtypes = [vp, C.c_double, C.c_int, C.POINTER(C.c_uint64), dp, dp, dp, dp,
                                     C.POINTER(C.c_int64)]
     L.lv_workspace_bytes.argtypes = [vp]
@@ -328,6 +334,29 @@ class Simulation:
             self._check(self.L.lv_render(self.h, C.byref(v), zbuf.data_ptr(), img.ctypes.data, 0),
                         "lv_render")
             self.stream.synchronize()
+            return img
+
+    def render_surface(self, width, height, palette, droplet=0xff302010, on_device=False):
+        """Equirectangular map of the NP intersections with the droplet surface (Fig. 2, left
+        panel) -> uint32[height, width] (numpy, or a torch tensor on the device)."""
+        import torch
+        m = LvSurfaceMap(int(width), int(height))
+        for a, c in enumerate(palette):
+            m.palette[a] = int(c)
+        m.droplet = int(droplet)
+        w_, h_ = max(int(width), 0), max(int(height), 0)
+        with torch.cuda.device(self.device):
+            scratch = torch.empty(w_ * h_ + w_ + h_ + 1, dtype=torch.int64, device=self.device)
+            scratch.record_stream(self.stream)
+            if on_device:
+                img = torch.empty((h_, w_), dtype=torch.int32, device=self.device)
+                img.record_stream(self.stream)
+                self._check(self.L.lv_render_surface(self.h, C.byref(m), scratch.data_ptr(),
+                                                     img.data_ptr(), 1), "lv_render_surface")
+                return img
+            img = np.zeros((h_, w_), dtype=np.uint32)
+            self._check(self.L.lv_render_surface(self.h, C.byref(m), scratch.data_ptr(),
+                                                 img.ctypes.data, 0), "lv_render_surface")
             return img
 
     def status(self) -> int:

@@ -773,6 +773,54 @@ int lv_render(lv_sim *s, const lv_view *view, void *zbuf_dev, uint32_t *rgba, in
     return LV_OK;
 }
 
+int lv_render_surface(lv_sim *s, const lv_surface_map *map, void *scratch_dev, uint32_t *rgba,
+                      int on_device)
+{
+    if (!s || !map || !scratch_dev || !rgba) return LV_E_ARG;
+    if (map->width < 1 || map->height < 1 || map->width > 8192 || map->height > 8192) return LV_E_ARG;
+    if (((uintptr_t)scratch_dev % 8) != 0) return LV_E_ARG;
+    if (!s->bound || !s->state_set) return LV_E_ORDER;
+    const int W = map->width, H = map->height;
+    // direction factors per column / row: fp64 libm, rounded once (include/lv.h)
+    struct Tab {                         // freed on every return path
+        float *p;
+        ~Tab() { free(p); }
+    } tabh{(float *)malloc(4 * (2 * (size_t)W + 2 * (size_t)H))};
+    float *tab = tabh.p;
+    if (!tab) return LV_E_NOMEM;
+    for (int px = 0; px < W; ++px) {
+        const double lam = -M_PI + (2.0 * M_PI) * (((double)px + 0.5) / (double)W);
+        tab[px] = (float)cos(lam);
+        tab[W + px] = (float)sin(lam);
+    }
+    for (int py = 0; py < H; ++py) {
+        const double phi = 0.5 * M_PI - M_PI * (((double)py + 0.5) / (double)H);
+        tab[2 * W + py] = (float)cos(phi);
+        tab[2 * W + H + py] = (float)sin(phi);
+    }
+    LvDevState st;
+    LV_CUDA(s, cudaMemcpyAsync(&st, s->bufs.st, sizeof(st), cudaMemcpyDeviceToHost, s->stream));
+    LV_CUDA(s, cudaStreamSynchronize(s->stream));
+    const double R = lv_radius_of(s->sched_mode, s->R0, s->R1, s->sched_steps, st.step);
+    const size_t n_px = (size_t)W * H;
+    unsigned long long *zbuf = (unsigned long long *)scratch_dev;
+    float *tab_dev = (float *)(zbuf + n_px);
+    LV_CUDA(s, cudaMemcpyAsync(tab_dev, tab, 4 * (2 * (size_t)W + 2 * (size_t)H), cudaMemcpyHostToDevice, s->stream));
+    uint32_t *drgba = rgba;
+    if (!on_device) LV_CUDA(s, cudaMallocAsync((void **)&drgba, 4 * n_px, s->stream));
+    cudaError_t e = lvk_render_surface(s->dev, s->bufs, map, R, tab_dev, zbuf, drgba, s->stream);
+    if (e == cudaSuccess && !on_device)
+        e = cudaMemcpyAsync(rgba, drgba, 4 * n_px, cudaMemcpyDeviceToHost, s->stream);
+    if (!on_device) {
+        cudaError_t e2 = cudaFreeAsync(drgba, s->stream);
+        if (e == cudaSuccess) e = e2;
+    }
+    // synchronise in both modes: `tab` is pageable host memory read by the stream
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s->stream);
+    if (e != cudaSuccess) return cuda_fail(s, e, "lv_render_surface");
+    return LV_OK;
+}
+
 int lv_get_status(lv_sim *s, uint32_t *status)
 {
     if (!s || !status) return LV_E_ARG;

@@ -158,6 +158,9 @@ cudaError_t lvk_clusters(const LvDev &P, const LvBufs &B, const float *rb2, cons
 // headless perspective view: zbuf W*H u64 (device scratch), rgba W*H u32 (device)
 cudaError_t lvk_render(const LvDev &P, const LvBufs &B, const lv_view *view, const float *rot9,
                        double R, unsigned long long *zbuf, uint32_t *rgba, cudaStream_t st);
+cudaError_t lvk_render_surface(const LvDev &P, const LvBufs &B, const lv_surface_map *map, double R,
+                               const float *tab_dev, unsigned long long *zbuf, uint32_t *rgba,
+                               cudaStream_t st);
 
 // FP32 FMA throughput probe (lv_measure_fp32_peak)
 cudaError_t lvk_fma_peak(float *scratch, int blocks, int iters, double *flops, cudaStream_t st);

@@ -537,7 +537,10 @@ k_pair_force_q(const __grid_constant__ LvDev P, const float4 *__restrict__ pos,
 #define LV_S_MINBLOCKS 4
 #endif
 constexpr int kSThreads = LV_S_THREADS;
-constexpr int kSegCap = 24;       // segments per lane between walks
+#ifndef LV_S_SEGCAP
+#define LV_S_SEGCAP 24
+#endif
+constexpr int kSegCap = LV_S_SEGCAP;       // segments per lane between walks
 constexpr int kSChunk = LV_S_CHUNK;
 
 template <int N> struct IntC { static constexpr int value = N; };
@@ -1463,6 +1466,84 @@ k_render_resolve(const LvViewDev V, const unsigned long long *__restrict__ zbuf,
     rgba[p] = c;
 }
 
+// ------------------------------------------------ surface map (NEXT-4), Fig. 2 left panel
+// "Projection of the microdroplet surface onto a plane", NP intersections with the surface
+// shown as circles elongated by the projection: an equirectangular map.  The
+// coverage test is the definition of include/lv.h evaluated literally (single fp32
+// operations); the lat/lon window each NP walks only has to CONTAIN its cap, so it is
+// computed with library transcendentals plus a margin and never decides a pixel.
+struct LvSurfDev {
+    int32_t width, height;
+    uint32_t palette[LV_MAX_TYPES];
+    uint32_t droplet;
+    float radius[LV_MAX_TYPES];
+    float R;
+};
+
+__global__ void __launch_bounds__(kThreads)
+k_surface_splat(int n, const LvSurfDev S, const float4 *__restrict__ pos,
+                const float *__restrict__ tab, unsigned long long *zbuf)
+{
+    const int i = blockIdx.x * kThreads + threadIdx.x;
+    if (i >= n) return;
+    const float4 p = pos[i];
+    const int a = __float_as_int(p.w);
+    const float r = S.radius[a], R = S.R;
+    const float r2 = __fmul_rn(r, r);
+    const int W = S.width, H = S.height;
+    const float *clon = tab, *slon = tab + W, *clat = tab + 2 * W, *slat = tab + 2 * W + H;
+    const float dist = sqrtf(p.x * p.x + p.y * p.y + p.z * p.z);
+    if (!(dist == dist) || !(fabsf(dist - R) <= r * 1.001f + 1e-5f * R)) return;   // cannot reach the surface
+    constexpr float kPi = 3.14159265358979f;
+    int y0 = 0, y1 = H - 1, x0 = 0, nx = W;
+    if (dist > 1e-6f * R) {
+        const float ca = fminf(1.0f, fmaxf(-1.0f, (R * R + dist * dist - r * r) / (2.0f * R * dist)));
+        const float alpha = acosf(ca) * 1.01f + 1e-4f;
+        const float phi0 = asinf(fminf(1.0f, fmaxf(-1.0f, p.z / dist)));
+        const float sc = (float)H / kPi;
+        y0 = max(0, (int)floorf((0.5f * kPi - (phi0 + alpha)) * sc - 0.5f) - 1);
+        y1 = min(H - 1, (int)ceilf((0.5f * kPi - (phi0 - alpha)) * sc - 0.5f) + 1);
+        if (fabsf(phi0) + alpha < 0.5f * kPi - 1e-3f) {
+            const float dl = asinf(fminf(1.0f, sinf(alpha) / cosf(phi0))) * 1.01f;
+            const float lam0 = atan2f(p.y, p.x);
+            const float xc = (lam0 + kPi) * (float)W / (2.0f * kPi) - 0.5f;
+            const float hw = dl * (float)W / (2.0f * kPi) + 2.0f;
+            if (2.0f * hw + 2.0f < (float)W) {
+                const int xa = (int)floorf(xc - hw), xb = (int)ceilf(xc + hw);
+                nx = xb - xa + 1;
+                x0 = ((xa % W) + W) % W;
+            }
+        }
+    }
+    const unsigned long long col = (unsigned long long)(S.palette[a] | 0xff000000u);
+    for (int py = y0; py <= y1; ++py) {
+        const float cl = clat[py], sl = slat[py];
+        const float sz = __fmul_rn(R, sl);
+        const float dz = __fsub_rn(sz, p.z);
+        const float dz2 = __fmul_rn(dz, dz);
+        int px = x0;
+        for (int k = 0; k < nx; ++k) {
+            const float sx = __fmul_rn(R, __fmul_rn(cl, clon[px]));
+            const float sy = __fmul_rn(R, __fmul_rn(cl, slon[px]));
+            const float dx = __fsub_rn(sx, p.x), dy = __fsub_rn(sy, p.y);
+            const float d2 = __fadd_rn(__fadd_rn(__fmul_rn(dx, dx), __fmul_rn(dy, dy)), dz2);
+            if (d2 < r2)
+                atomicMin(zbuf + (size_t)py * W + px, ((unsigned long long)__float_as_uint(d2) << 32) | col);
+            px = px + 1 == W ? 0 : px + 1;
+        }
+    }
+}
+
+__global__ void __launch_bounds__(kThreads)
+k_surface_resolve(int n_px, uint32_t droplet, const unsigned long long *__restrict__ zbuf,
+                  uint32_t *__restrict__ rgba)
+{
+    const int p = blockIdx.x * kThreads + threadIdx.x;
+    if (p >= n_px) return;
+    const unsigned long long k = zbuf[p];
+    rgba[p] = k == 0xffffffffffffffffull ? droplet : (uint32_t)k;
+}
+
 inline int blocks_for(int n) { return n > 0 ? (n + kThreads - 1) / kThreads : 1; }
 
 }  // namespace
@@ -1707,6 +1788,27 @@ cudaError_t lvk_render(const LvDev &P, const LvBufs &B, const lv_view *view, con
     k_render_clear<<<blocks_for(n_px), kThreads, 0, st>>>(n_px, zbuf);
     if (P.n > 0) k_render_splat<<<blocks_for(P.n), kThreads, 0, st>>>(P.n, V, B.posA, zbuf);
     k_render_resolve<<<blocks_for(n_px), kThreads, 0, st>>>(V, zbuf, rgba);
+    return cudaGetLastError();
+}
+
+cudaError_t lvk_render_surface(const LvDev &P, const LvBufs &B, const lv_surface_map *map, double R,
+                               const float *tab_dev, unsigned long long *zbuf, uint32_t *rgba,
+                               cudaStream_t st)
+{
+    LvSurfDev S;
+    memset(&S, 0, sizeof(S));
+    S.width = map->width;
+    S.height = map->height;
+    for (int a = 0; a < LV_MAX_TYPES; ++a) {
+        S.palette[a] = map->palette[a];
+        S.radius[a] = (float)P.radius_d[a];
+    }
+    S.droplet = map->droplet;
+    S.R = (float)R;
+    const int n_px = map->width * map->height;
+    k_render_clear<<<blocks_for(n_px), kThreads, 0, st>>>(n_px, zbuf);
+    if (P.n > 0) k_surface_splat<<<blocks_for(P.n), kThreads, 0, st>>>(P.n, S, B.posA, tab_dev, zbuf);
+    k_surface_resolve<<<blocks_for(n_px), kThreads, 0, st>>>(n_px, map->droplet, zbuf, rgba);
     return cudaGetLastError();
 }
 

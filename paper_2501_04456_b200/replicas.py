@@ -49,3 +49,62 @@ def reduce_timing(elapsed_ms: float, units: float, device="cpu") -> Tuple[float,
     dist.all_reduce(t, op=dist.ReduceOp.MAX)
     dist.all_reduce(u, op=dist.ReduceOp.SUM)
     return float(t.item()), float(u.item())
+
+
+def _check_cuda_extension() -> None:
+    """ReplicaSet is a product path: it fails loudly without the CUDA library
+    (no CPU fallback)."""
+    from . import binding
+    binding.load()
+
+
+class ReplicaSet:
+    """R independent replicas of one workload on ONE GPU, each an `lv_sim`
+    handle on its own CUDA stream ("batched replicas of
+    small droplets" -- a C1- or Table-1-sized droplet, fills a
+    fraction of a B200, and the paper's use is many scenarios / seeds for
+    hypothesis testing).  `step(n)` enqueues the n graph
+    replays of every replica in slices, round robin, so that every stream
+    always has work queued and the kernels of different replicas overlap on
+    the SMs.  There is no coupling between replicas: replica r of the set
+    is bit-identical to the same workload stepped alone
+    (tests/test_gpu_parity.py::test_replica_set_equals_solo_runs)."""
+
+    def __init__(self, make_workload, n_replicas: int, base_seed: int, device: str = "cuda:0",
+                 cells_per_cut=None, options=None, neighbour_list=None, slice_steps: int = 50):
+        _check_cuda_extension()
+        from . import binding
+        if n_replicas < 1:
+            raise ValueError("n_replicas must be >= 1")
+        self.slice_steps = int(slice_steps)
+        self.workloads = [make_workload(replica_seed(base_seed, r)) for r in range(n_replicas)]
+        self.sims = [binding.Simulation.from_workload(
+            w, cells_per_cut=cells_per_cut if cells_per_cut is not None else w.tuned_cells_per_cut,
+            device=device, options=options, neighbour_list=neighbour_list) for w in self.workloads]
+
+    def __len__(self) -> int:
+        return len(self.sims)
+
+    @property
+    def n_particles(self) -> int:
+        return sum(w.n for w in self.workloads)
+
+    def step(self, n: int = 1) -> None:
+        done = 0
+        while done < n:
+            k = min(self.slice_steps, n - done)
+            for s in self.sims:
+                s.step(k)
+            done += k
+
+    def synchronize(self) -> None:
+        for s in self.sims:
+            s.synchronize()
+
+    def get_state(self, r: int, **kw):
+        return self.sims[r].get_state(**kw)
+
+    def close(self) -> None:
+        for s in self.sims:
+            s.close()
+        self.sims = []

@@ -306,6 +306,34 @@ def test_split_invariance_and_roundtrip(B):
         s.close()
 
 
+def test_replica_set_equals_solo_runs(B, orc):
+    """NEXT-3 batched replicas: R small droplets stepped concurrently on R streams of one GPU
+    are each bit-identical to the same workload stepped alone (no coupling between
+    replicas), differ from one another (distinct seeds), and replica 0 still tracks the oracle."""
+    from paper_2501_04456_b200 import replicas
+    mk = lambda seed: W.make_workload("C1", 1024, seed=seed)
+    rs = replicas.ReplicaSet(mk, 5, base_seed=77, slice_steps=7)
+    assert len(rs) == 5 and rs.n_particles == 5 * 1024
+    rs.step(40)
+    rs.synchronize()
+    got = [rs.get_state(r) for r in range(5)]
+    for r in range(5):
+        solo = B.Simulation.from_workload(rs.workloads[r], cells_per_cut=rs.workloads[r].tuned_cells_per_cut)
+        solo.step(40)
+        ref = solo.get_state()
+        for u, v in zip(got[r][:3], ref[:3]):
+            assert np.array_equal(u, v)
+        assert got[r][3:] == ref[3:]
+        solo.close()
+    assert not np.array_equal(got[0][0], got[1][0])
+    w0 = rs.workloads[0]
+    p = orc.params_from_workload(w0)
+    xo, vo, bad = orc.step(p, w0.pos, w0.vel, w0.type, step0=0, nsteps=40)
+    assert bad == 0
+    assert np.linalg.norm(got[0][0].astype(np.float64) - xo, axis=1).max() <= 1e-3 * got[0][3]
+    rs.close()
+
+
 def test_restart_continues_within_tolerance(B):
     """Stop, save, restart (PAPER.md:84): same noise (keyed on id and step);
     only the summation order changes, so the continuation agrees to rounding."""
