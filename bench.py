@@ -518,7 +518,7 @@ def main():
     ap.add_argument("--start-step", type=int, default=0)
     ap.add_argument("--cells-per-cut", type=int, nargs="*", default=None)
     ap.add_argument("--force-kernel", type=int, default=None,
-                    help="lv_set_option(LV_OPT_FORCE_KERNEL): 0 simple, 1 queued, 2 segments")
+                    help="lv_set_option(LV_OPT_FORCE_KERNEL): 0 simple, 1 queued, 2 segments (default), 3 packed f32x2")
     ap.add_argument("--neighbour-list", type=float, nargs=2, default=None, metavar=("SKIN", "CAP"),
                     help="lv_set_neighbour_list: time the skin-list variant instead of the per-step rebuild")
     ap.add_argument("--no-variants", action="store_true", help="skip the skin-list variant")
