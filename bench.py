@@ -11,13 +11,18 @@ centrifugal, shrinking interface), the configuration with the N = 2.5e5 the
 metric is quoted on; inputs are seeded and synthetic (workloads.py).
 
 Own arm (--impl lv, default):
-  value       whole-job particle-steps/s, state resident in HBM, K timed steps,
-              device time from CUDA events recorded by the library on its own
-              stream around every step (and every stage), L2 flushed (256 MiB
-              memset) between timed steps, max over ranks.
-  roofline    the pair-force kernel (dominant): algorithmic FP32 flops per
-              launch / its average CUDA-event duration inside the same timed
-              region, against the FP32 FMA peak derived in DESIGN.md.
+  value       whole-job particle-steps/s, state resident in HBM, K timed steps of
+              the product path (lv_step(1) = one CUDA-graph replay of the whole
+              step), device time from a CUDA event pair on the library's stream
+              around every step, L2 flushed (256 MiB memset) between timed
+              steps, max over ranks.
+  stage_ms_per_step / roofline
+              the K steps that follow are launched kernel by kernel with an event
+              after every stage (lv_stage_timing; ~2.5 us of event overhead per
+              stage, hence not the headline): the breakdown, and the pair-force
+              kernel's average duration for the roofline -- algorithmic FP32
+              flops per launch / that duration, against the FP32 FMA peak
+              derived in DESIGN.md.
   resident    the same K steps as one lv_step(K) graph replay without flushes
               (how a simulation actually runs: the 8 MB state stays in L2).
   e2e         set_state(host) + lv_step(1) + get_state(host) per step through
@@ -146,6 +151,22 @@ def timed_steps(sim, torch, flush, k):
     return stages, tot
 
 
+def timed_steps_product(sim, torch, flush, k):
+    """k steps through the product path -- lv_step(1) = one CUDA-graph replay of the whole
+    step -- L2 flushed between steps, one CUDA event pair per step on the library's stream
+    (the flush is outside the pairs).  -> step ms sum."""
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(k)]
+    with torch.cuda.stream(sim.stream):
+        for e0, e1 in ev:
+            if flush is not None:
+                flush.zero_()
+            e0.record()
+            sim.step(1)
+            e1.record()
+    sim.synchronize()
+    return sum(e0.elapsed_time(e1) for e0, e1 in ev)
+
+
 def inrange_pairs(sim):
     sim.compute_forces()
     _, cnt = sim.get_forces()
@@ -154,9 +175,10 @@ def inrange_pairs(sim):
 
 def measure_point(sim, torch, flush, w, steps, warmup):
     """One measurement of the resident-state throughput at the current step."""
-    timed_steps(sim, torch, flush, max(warmup, 1))
+    timed_steps_product(sim, torch, flush, max(warmup, 1))
+    tot = timed_steps_product(sim, torch, flush, steps)
     p0 = inrange_pairs(sim)
-    stages, tot = timed_steps(sim, torch, flush, steps)
+    stages, _ = timed_steps(sim, torch, flush, steps)
     p1 = inrange_pairs(sim)
     return stages, tot, 0.5 * (p0 + p1)
 
@@ -193,19 +215,24 @@ def run_lv(args):
     n_sms = torch.cuda.get_device_properties(device).multi_processor_count
     fma_tflops = sim.measure_fp32_peak()
 
-    # ---- timed region: K steps, events on the library's stream -------------
-    timed_steps(sim, torch, flush, max(args.warmup, 3))
-    pairs0 = inrange_pairs(sim)
+    # ---- timed region: K steps of the product path (graph replay), events on the
+    # library's stream around every step --------------------------------------
+    timed_steps_product(sim, torch, flush, max(args.warmup, 3))
     sampler = ClockSampler(visible_gpu_index(local_rank))
     replicas.barrier()
     torch.cuda.synchronize()
     sampler.start()
     t_wall0 = time.perf_counter()
-    stages, tot_ms = timed_steps(sim, torch, flush, args.steps)
+    tot_ms = timed_steps_product(sim, torch, flush, args.steps)
     torch.cuda.synchronize()
     wall_s = time.perf_counter() - t_wall0
     clocks = sampler.finish()
     replicas.barrier()
+    # ---- stage pass: the next K steps launched kernel by kernel with an event after every
+    # stage (lv_stage_timing); the event records cost ~2.5 us per stage, so this pass is
+    # the breakdown and the source of the pair-force kernel time, not the headline
+    pairs0 = inrange_pairs(sim)
+    stages, stage_tot_ms = timed_steps(sim, torch, flush, args.steps)
     pairs1 = inrange_pairs(sim)
     launches_per_step = sim.launches_per_step()
 
@@ -232,10 +259,11 @@ def run_lv(args):
                                               neighbour_list=(skin, cap))
         if args.start_step > 0:
             vs.step(args.start_step)
-        timed_steps(vs, torch, flush, max(args.warmup, 3))
+        timed_steps_product(vs, torch, flush, max(args.warmup, 3))
         r0 = vs.rebuild_count()
-        vstages, vtot = timed_steps(vs, torch, flush, args.steps)
+        vtot = timed_steps_product(vs, torch, flush, args.steps)
         r1 = vs.rebuild_count()
+        vstages, _ = timed_steps(vs, torch, flush, args.steps)
         vs.step(max(args.warmup, 3))
         vs.synchronize()
         e0.record(vs.stream)
@@ -379,7 +407,9 @@ def run_lv(args):
         "algorithmic_flops_per_launch": flops,
         "in_range_ordered_pairs": pairs, "flop_per_pair": FLOP_PER_PAIR,
         "kernel_ms": force_ms,
-        "share_of_step": stages["pair_force"] / tot_ms,
+        "share_of_step": stages["pair_force"] / stage_tot_ms,
+        "kernel_ms_source": "stage-event pass over the K steps that follow the headline region "
+                            "(same workload, kernels launched one by one with an event after each stage)",
         "hbm_algorithmic_gbs": 32.0 * n / (force_ms * 1e-3) * 1e-9,
         "hbm_peak_gbs": pk["hbm_gbs"],
     }
@@ -396,11 +426,12 @@ def run_lv(args):
                        2 if args.force_kernel is None else args.force_kernel],
                    "replicas": world, "parallelism": "independent replicas, no collective",
                    "l2": "flushed between timed steps (256 MiB memset on the same stream)",
-                   "timing": "CUDA events on the library's stream around every step; sum over K"},
+                   "timing": "lv_step(1) = one CUDA-graph replay per step; a CUDA event pair on the library's stream around every step (the flush outside it); sum over K"},
         "clocks": clocks,
         "gpu_launches": launches_per_step * args.steps,
         "launches_per_step": launches_per_step,
         "stage_ms_per_step": {k: v / args.steps for k, v in stages.items()},
+        "stage_pass_ms_per_step": stage_tot_ms / args.steps,
         "wall_s_timed_region": wall_s,
         "roofline": roofline,
         "variants": variants,
