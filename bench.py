@@ -407,7 +407,8 @@ def run_lv(args):
         "algorithmic_flops_per_launch": flops,
         "in_range_ordered_pairs": pairs, "flop_per_pair": FLOP_PER_PAIR,
         "kernel_ms": force_ms,
-        "share_of_step": stages["pair_force"] / stage_tot_ms,
+        "share_of_step": stages["pair_force"] / tot_ms,          # against the graph-replayed (headline) step
+        "share_of_stage_pass": stages["pair_force"] / stage_tot_ms,   # that pass carries event overhead
         "kernel_ms_source": "stage-event pass over the K steps that follow the headline region "
                             "(same workload, kernels launched one by one with an event after each stage)",
         "hbm_algorithmic_gbs": 32.0 * n / (force_ms * 1e-3) * 1e-9,
