@@ -122,6 +122,16 @@ def _spec(name: str) -> Workload:
                         tuned_neighbour_list=(0.4, 128))
     # ---- paper-shaped scenarios (Table 1) in reduced units; synthetic
     # stand-ins: the authors' parameter files are not available
+    if name == "T8":
+        # edge case, not a BASELINE config: the maximum number of coexisting types (T = 8 =
+        # LV_MAX_TYPES), eight sizes, alternating charges, every force term switched on
+        s = [1.0, 1.2, 1.4, 1.6, 1.8, 2.0, 2.2, 2.4]
+        return Workload("T8", 12000, s, [1.0, 2.0, 0.5, 1.5, 3.0, 0.7, 1.2, 2.5],
+                        [0.0, 1.0, -1.0, 0.5, -0.5, 0.0, 2.0, -2.0], _mass(s), [100.0] * 8, [1.5] * 8,
+                        [0.2, 0.15, 0.15, 0.1, 0.1, 0.1, 0.1, 0.1], kT=1.0, dt=0.002, cut_factor=3.0,
+                        coulomb_k=0.7, g=0.01, omega2=(2.5e-5, 2.5e-5, 0.0), wall_mode=WALL_ONESIDED,
+                        sched_mode=SCHED_LINEAR, R0=45.0, R1=25.0, sched_steps=5000, seed=21,
+                        steps=5000, init="ball", tuned_cells_per_cut=[1] * 8)
     if name == "P1":
         # row "1" (Fig. 2, 7): R0 = 20 um, r_NP = 0.5 um -> sigma = 1, R0 = 20; 10^4 neutral NPs,
         # LJ only, range 4 (r_A + r_B), no evaporation, random tumbling =
@@ -239,7 +249,7 @@ def fcc_ball(rng, n, sigma, R, jitter=0.05):
 
 def make_workload(name: str, n: Optional[int] = None, state: bool = True,
                   seed: Optional[int] = None) -> Workload:
-    """BASELINE config `name` ("C1".."C5") or paper-shaped scenario ("P1", "P8").  With n given, a scaled-down (or
+    """BASELINE config `name` ("C1".."C5"), paper-shaped scenario ("P1", "P8") or the eight-type edge case ("T8").  With n given, a scaled-down (or
     up) copy at the same volume fractions: radii scale as (n/N)^(1/3).  `seed`
     overrides the configuration's seed (independent replicas)."""
     w = _spec(name)

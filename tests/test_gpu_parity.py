@@ -33,6 +33,8 @@ CASES = [          # (config, n or None for full size, cells_per_cut)
     ("C4", 20000, None),
     ("C4", 19999, [2]),
     ("C5", 20001, None),
+    ("T8", None, None),                     # LV_MAX_TYPES coexisting types
+    ("T8", 5003, [1, 2, 1, 2, 1, 2, 1, 3]),
 ]
 
 _cache = {}
@@ -144,7 +146,8 @@ def vel_pos_check(w, p_orc, xo, vo, xg, vg, S_pair, R):
     assert dx.max() / R <= 1e-5
 
 
-@pytest.mark.parametrize("name,n", [("C1", None), ("C2", 8192), ("C3", 20000), ("C4", 20000), ("C5", 20001)])
+@pytest.mark.parametrize("name,n", [("C1", None), ("C2", 8192), ("C3", 20000), ("C4", 20000), ("C5", 20001),
+                                    ("T8", None)])
 def test_one_step(B, orc, name, n):
     w = workload(name, n)
     p = orc.params_from_workload(w)
@@ -182,7 +185,7 @@ def test_one_step_moving_interface_near_wall(B, orc):
     sim.close()
 
 
-@pytest.mark.parametrize("name,n", [("C1", None), ("C2", 8192), ("C4", 8000)])
+@pytest.mark.parametrize("name,n", [("C1", None), ("C2", 8192), ("C4", 8000), ("T8", 6000)])
 def test_hundred_steps(B, orc, name, n):
     w = workload(name, n)
     p = orc.params_from_workload(w)
