@@ -132,7 +132,9 @@ Layout layout_of(const lv_sim *s)
     L.sort_temp_bytes = lvs_temp_bytes(s->n, s->sort_end_bit);
     L.sort_temp = take(L.sort_temp_bytes);
     L.st = take(sizeof(LvDevState));
-    L.staging = take(28 * n);
+    // host-transfer staging (28 B per NP); also the scratch of the observables, so never
+    // smaller than their largest histogram (8 * 8192 + 64 B)
+    L.staging = take(28 * n > 65600 ? 28 * n : 65600);
     L.posP = take(16 * (n + 4));   // pair-interleaved copy of posB + dummy slots (LV_FORCE_PACKED)
     const size_t n_warps = ((n + 127) / 128) * 4;      // warps of the 128-thread force launches
     L.list = take(s->list_cap > 0 ? 4 * n_warps * 32 * (size_t)s->list_cap : 0);
@@ -597,7 +599,8 @@ constexpr int kMaxObsBins = 8192;
 int obs_scratch(lv_sim *s, int n_bins, unsigned long long **hist, double **sums)
 {
     const size_t need = 8 * (size_t)n_bins + 64;
-    if (need > 28 * (size_t)(s->n > 0 ? s->n : 1)) return LV_E_ARG;
+    const size_t have = 28 * (size_t)s->n > 65600 ? 28 * (size_t)s->n : 65600;
+    if (need > have) return LV_E_ARG;
     *hist = (unsigned long long *)s->bufs.staging;
     *sums = (double *)(s->bufs.staging + 8 * (size_t)n_bins);
     LV_CUDA(s, cudaMemsetAsync(s->bufs.staging, 0, need, s->stream));
@@ -721,7 +724,7 @@ int lv_observe_clusters(lv_sim *s, double bond_factor, int32_t *labels, int64_t 
     s->force_order_b = true;
     // scratch in the staging area: 3 uint32[n] | int32 labels[n] | 34 u64 statistics
     const size_t n = (size_t)s->n;
-    if (28 * n < 16 * n + 34 * 8 + 8) return LV_E_ARG;
+    if ((28 * n > 65600 ? 28 * n : 65600) < 16 * n + 34 * 8 + 8) return LV_E_ARG;   // staging >= 65600 B
     uint32_t *scratch = (uint32_t *)s->bufs.staging;
     int32_t *dlab = (int32_t *)(s->bufs.staging + 12 * n);
     unsigned long long *dst = (unsigned long long *)(s->bufs.staging + ((16 * n + 7) / 8) * 8);

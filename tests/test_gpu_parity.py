@@ -429,6 +429,40 @@ def test_tiny_and_empty(B, orc, n):
     sim.close()
 
 
+@pytest.mark.parametrize("n", [0, 1, 2])
+def test_tiny_and_empty_observables_and_views(B, orc, n):
+    """The rows built after the step (observables, aggregates, both views) on empty and tiny
+    inputs: no crash, and the same answers as the oracle."""
+    from oracle import observables as O
+    x = np.array([[5.6, 0.0, 0.0], [4.5, 0.0, 0.0]], np.float32)[:n]     # one NP in the interface, a bonded pair
+    t = np.zeros(n, np.int32)
+    sim = B.Simulation(n, 1, 5, 0.005)
+    ga, gb = B.langevin_coeffs(1.0, 1.0, 1.0, 0.005)
+    sim.set_types([dict(sigma=1.0, eps=1.0, mass=1.0, wall_k=100.0, drag_a=ga, kick_b=gb)], cut_factor=2.5)
+    sim.set_droplet_schedule(B.SCHED_CONST, 6.0)
+    sim.bind()
+    sim.set_state(x, np.zeros((n, 3), np.float32), t, 0)
+    hist, g = sim.observe_rdf(0.1, 25)
+    assert hist.sum() == (2 if n == 2 else 0)            # the ordered pair at r = 1.1, both ways
+    assert np.array_equal(hist, orc.rdf_hist(x, 0.1, 25))
+    rad = sim.observe_radial(0.5, 16)
+    assert rad["hist"].sum() == n and rad["n_surf"] == (1 if n else 0)   # |x| = 5.6 > R - 2 r
+    cl = sim.observe_clusters(1.5)
+    assert cl["n_clusters"] == (1 if n else 0) and cl["largest"] == n
+    if n:
+        assert np.array_equal(cl["labels"], np.zeros(n, np.int32))
+        assert np.array_equal(O.cluster_labels(x.astype(np.float64), t, [1.0]), np.zeros(n))
+    pal = [0x00ff8040]
+    img = sim.render(30.0, 200.0, 0.2, 0.1, 64, 48, pal, 0xff000000, 0xff201008)
+    ref = orc.render(x, t, [0.5], 6.0, 30.0, 200.0, 0.2, 0.1, 64, 48, pal, 0xff000000, 0xff201008)
+    assert np.array_equal(img, ref)
+    smap = sim.render_surface(90, 45, pal, 0xff201008)
+    sref = orc.render_surface(x, t, [0.5], 6.0, 90, 45, pal, 0xff201008)
+    assert np.array_equal(smap, sref)
+    assert ((smap != 0xff201008).sum() > 0) == (n >= 1)
+    sim.close()
+
+
 def test_status_flags(B):
     w = workload("C1", None)
     sim = B.Simulation.from_workload(w, load_state=False)
