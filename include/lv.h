@@ -218,8 +218,7 @@ int lv_get_forces(lv_sim *s, float *force_xyz, int32_t *neigh_count, int on_devi
 
 /* ---- observables of the paper on the device ----------------
  * Shell index of a distance (fp32 contract #4): (int) fl32(sqrt(r2) * fl32(1/dr))
- * with r2 as in the in-range predicate; counted iff < n_bins (1..8192, and
- * 8 n_bins + 64 <= 28 n).  All outputs are host memory, written; any may be NULL.
+ * with r2 as in the in-range predicate; counted iff < n_bins (1..8192).  All outputs are host memory, written; any may be NULL.
  * Both calls synchronise the stream and leave the state unchanged.
  *
  * lv_observe_rdf: radial distribution function, Eq. 6.  hist[k] =
