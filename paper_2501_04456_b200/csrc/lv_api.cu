@@ -860,6 +860,7 @@ int lv_get_state(lv_sim *s, float *pos_xyz, float *vel_xyz, int32_t *type, doubl
     LV_CUDA(s, cudaStreamSynchronize(s->stream));
     if (step) *step = (int64_t)h.step;
     if (R) *R = lv_radius_of(s->sched_mode, s->R0, s->R1, s->sched_steps, h.step);
+    if (h.status & LV_ST_BAD_TYPE) return LV_E_ARG;
     if (h.status & LV_ST_NONFINITE) return LV_E_NONFINITE;
     return (h.status & LV_ST_LIST_OVERFLOW) ? LV_E_CAPACITY : LV_OK;
 }

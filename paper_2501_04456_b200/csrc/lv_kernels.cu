@@ -1084,19 +1084,24 @@ k_update(const __grid_constant__ LvDev P, const float4 *__restrict__ posB_,
 
 // ------------------------------------------------- state in / out (by id)
 __global__ void __launch_bounds__(kThreads)
-k_pack_state(int n, const float *__restrict__ pos, const float *__restrict__ vel,
+k_pack_state(int n, int n_types, const float *__restrict__ pos, const float *__restrict__ vel,
              const int32_t *__restrict__ type, float4 *__restrict__ posA,
              float4 *__restrict__ velA, LvDevState *st, long long step)
 {
     int i = blockIdx.x * kThreads + threadIdx.x;
     if (i == 0) {
-        st->step = step; st->status = 0u; st->ticket = 0u;
+        st->step = step; st->ticket = 0u;       // status: cleared by lvk_pack_state before the launch
         st->rebuild[step & 1] = 1u;            // skin list: the first step builds it
         st->rebuild[(step + 1) & 1] = 0u;
         st->n_rebuilds = 0u;
     }
     if (i >= n) return;
-    posA[i] = make_float4(pos[3 * i], pos[3 * i + 1], pos[3 * i + 2], __int_as_float(type[i]));
+    int a = type[i];
+    if ((unsigned)a >= (unsigned)n_types) {       // would index the type tables out of range
+        a = 0;
+        atomicOr(&st->status, LV_ST_BAD_TYPE);
+    }
+    posA[i] = make_float4(pos[3 * i], pos[3 * i + 1], pos[3 * i + 2], __int_as_float(a));
     velA[i] = make_float4(vel[3 * i], vel[3 * i + 1], vel[3 * i + 2], __uint_as_float((uint32_t)i));
 }
 
@@ -1686,7 +1691,10 @@ cudaError_t lvk_update_list(const LvDev &P, const LvBufs &B, cudaStream_t st)
 cudaError_t lvk_pack_state(const LvDev &P, const LvBufs &B, const float *pos, const float *vel,
                            const int32_t *type, long long step, cudaStream_t st)
 {
-    k_pack_state<<<blocks_for(P.n), kThreads, 0, st>>>(P.n, pos, vel, type, B.posA, B.velA, B.st, step);
+    // cleared ahead of the kernel: its threads raise LV_ST_BAD_TYPE with atomicOr
+    cudaError_t e = cudaMemsetAsync(&B.st->status, 0, sizeof(B.st->status), st);
+    if (e != cudaSuccess) return e;
+    k_pack_state<<<blocks_for(P.n), kThreads, 0, st>>>(P.n, P.n_types, pos, vel, type, B.posA, B.velA, B.st, step);
     return cudaGetLastError();
 }
 

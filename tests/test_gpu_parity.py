@@ -494,6 +494,27 @@ def test_status_flags(B):
     sim.close()
 
 
+def test_type_out_of_range_is_reported(B):
+    """An NP type outside [0, n_types) would index the type tables out of range: it is loaded
+    as type 0, LV_ST_BAD_TYPE is raised and lv_get_state returns LV_E_ARG."""
+    w = workload("C2", 8192)
+    sim = B.Simulation.from_workload(w, load_state=False)
+    t = w.type.copy()
+    t[17] = 2
+    t[4000] = -1
+    sim.set_state(w.pos, w.vel, t, 0)
+    sim.step(2)
+    assert sim.status() & 8
+    with pytest.raises(B.LvError) as ei:
+        sim.get_state()
+    assert ei.value.code == -1
+    sim.set_state(w.pos, w.vel, w.type, 0)      # a valid state clears the flag
+    sim.step(2)
+    assert sim.status() == 0
+    sim.get_state()
+    sim.close()
+
+
 def test_wall_window_mode_and_r2law(B, orc):
     w = W.make_workload("C1", None)
     w.wall_mode = W.WALL_WINDOW
