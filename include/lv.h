@@ -194,7 +194,7 @@ int lv_bind(lv_sim *s, void *workspace_dev, size_t workspace_bytes, void *cuda_s
  * vel_xyz: [n][3] fp32; type: [n] int32 in [0, n_types); all three host
  * (on_device = 0) or all device (on_device = 1); copied.  NP id = row index.
  * step = index of the next step to take.  Synchronises the stream when the
- * sources are host buffers. * A type outside [0, n_types) is loaded as type 0 and raises LV_ST_BAD_TYPE (checked on the
+ * sources are host buffers.  A type outside [0, n_types) is loaded as type 0 and raises LV_ST_BAD_TYPE (checked on the
  * device: the call stays asynchronous); lv_get_state then returns LV_E_ARG. */
 int lv_set_state(lv_sim *s, const float *pos_xyz, const float *vel_xyz, const int32_t *type,
                  int64_t step, int on_device);
