@@ -406,6 +406,9 @@ def run_lv(args):
                        f"(DESIGN.md); measured FMA microkernel {fma_tflops:.1f} TFLOP/s",
         "algorithmic_flops_per_launch": flops,
         "in_range_ordered_pairs": pairs, "flop_per_pair": FLOP_PER_PAIR,
+        # SURVEY 8(d) quotes "~33" flops per in-range pair (distance test + force); DESIGN.md sec. 7
+        # counts 22 (Coulomb's 4 not counted).  The fraction at the survey's figure, for comparison:
+        "frac_at_33_flop_per_pair": 33.0 / FLOP_PER_PAIR * achieved / peak_tflops,
         "kernel_ms": force_ms,
         "share_of_step": stages["pair_force"] / tot_ms,          # against the graph-replayed (headline) step
         "share_of_stage_pass": stages["pair_force"] / stage_tot_ms,   # that pass carries event overhead
