@@ -151,6 +151,14 @@ int lv_set_grid(lv_sim *s, const int32_t *cells_per_cut);
  *                        dilute ones); LV_FORCE_QUEUED: row-by-row lock step with
  *                        per-thread in-range queues; LV_FORCE_SIMPLE: the first kernel.
  *                        The last two are kept as measured baselines.
+ *                        LV_FORCE_TILE: shared candidate stream for dense states -- a warp
+ *                        owns a tile of 32 / S consecutive sorted targets of one type, the
+ *                        stencil rows around the tile's bounding box are staged into shared
+ *                        memory by 1-D bulk copies (TMA), and S lanes per target walk the
+ *                        same staged stream (steps i-ii).
+ *   LV_OPT_TILE_SUBSTREAMS  S of LV_FORCE_TILE: 1, 2, 4 (default), 8, 16 or 32 lanes per target.
+ *   LV_OPT_TILE_SPAN     cells along x (of the targets' own grid) a tile may extend beyond
+ *                        the cell of its first target; -1 (default): cells_per_cut - 1.
  * Every setting gives bit-identical permutations, offsets and neighbour counts;
  * forces agree to rounding. */
 #define LV_OPT_SORT          1
@@ -161,6 +169,9 @@ int lv_set_grid(lv_sim *s, const int32_t *cells_per_cut);
 #define LV_FORCE_QUEUED      1
 #define LV_FORCE_SEGMENTS    2
 #define LV_FORCE_PACKED      3
+#define LV_FORCE_TILE        4
+#define LV_OPT_TILE_SUBSTREAMS 3
+#define LV_OPT_TILE_SPAN       4
 int lv_set_option(lv_sim *s, int option, int value);
 
 /* Optional throughput variant: a persistent "skin" neighbour

@@ -37,6 +37,8 @@ struct lv_sim {
     int32_t cells_per_cut[LV_MAX_TYPES];
     int sort_mode = LV_SORT_COUNTING;
     int force_kernel = LV_FORCE_SEGMENTS;
+    int tile_substreams = 4;        // LV_OPT_TILE_SUBSTREAMS: lanes per target of LV_FORCE_TILE
+    int tile_span = -1;             // LV_OPT_TILE_SPAN: cells along x a tile may span beyond its first (-1: k_a - 1)
     lv_grid_info grid;
     int sort_end_bit = 1;
     size_t ws_bytes = 0;
@@ -185,6 +187,8 @@ void derive_tables(lv_sim *s)
         d.grid[a].G = s->grid.G[a];
         d.grid[a].base = s->grid.base[a];
     }
+    for (int a = 0; a < T; ++a)
+        d.tile_cells[a] = s->tile_span >= 0 ? s->tile_span : s->cells_per_cut[a] - 1;
     d.dt = (float)s->dt;
     d.g = (float)s->g;
     for (int k = 0; k < 3; ++k) d.om2[k] = (float)s->om2[k];
@@ -238,13 +242,16 @@ int enqueue_stage(lv_sim *s, int stage, bool list_step = false)
     case 2:
         if (counting) {
             LV_CUDA(s, lvk_place(s->dev, s->bufs, false, s->stream));
-            LV_CUDA(s, lvk_rank_gather(s->dev, s->bufs, s->force_kernel == LV_FORCE_PACKED, false, s->stream));
+            LV_CUDA(s, lvk_rank_gather(s->dev, s->bufs, s->force_kernel == LV_FORCE_PACKED || s->force_kernel == LV_FORCE_TILE, false, s->stream));
         } else {
-            LV_CUDA(s, lvk_bounds_scatter(s->dev, s->bufs, s->force_kernel == LV_FORCE_PACKED, s->stream));
+            LV_CUDA(s, lvk_bounds_scatter(s->dev, s->bufs, s->force_kernel == LV_FORCE_PACKED || s->force_kernel == LV_FORCE_TILE, s->stream));
         }
         break;
     case 3:
-        LV_CUDA(s, lvk_pair_force(s->dev, s->bufs, s->force_kernel, s->stream));
+        if (s->force_kernel == LV_FORCE_TILE)
+            LV_CUDA(s, lvk_pair_force_tile(s->dev, s->bufs, s->tile_substreams, lvk_any_charge(s->dev), s->stream));
+        else
+            LV_CUDA(s, lvk_pair_force(s->dev, s->bufs, s->force_kernel, s->stream));
         break;
     default:
         LV_CUDA(s, lvk_update(s->dev, s->bufs, counting, s->stream));
@@ -444,8 +451,16 @@ int lv_set_option(lv_sim *s, int option, int value)
         s->sort_mode = value;
         return LV_OK;
     case LV_OPT_FORCE_KERNEL:
-        if (value < LV_FORCE_SIMPLE || value > LV_FORCE_PACKED) return LV_E_ARG;
+        if (value < LV_FORCE_SIMPLE || value > LV_FORCE_TILE) return LV_E_ARG;
         s->force_kernel = value;
+        return LV_OK;
+    case LV_OPT_TILE_SUBSTREAMS:
+        if (value < 1 || value > 32 || (value & (value - 1)) != 0) return LV_E_ARG;
+        s->tile_substreams = value;
+        return LV_OK;
+    case LV_OPT_TILE_SPAN:
+        if (value < -1 || value > 1024) return LV_E_ARG;
+        s->tile_span = value;
         return LV_OK;
     default:
         return LV_E_ARG;
@@ -514,6 +529,7 @@ int lv_bind(lv_sim *s, void *workspace_dev, size_t workspace_bytes, void *cuda_s
     s->ws_bytes = L.total;
     s->stream = (cudaStream_t)cuda_stream;
     derive_tables(s);
+    LV_CUDA(s, lvk_tile_prepare());
     LV_CUDA(s, cudaMemsetAsync(B.st, 0, sizeof(LvDevState), s->stream));
     // the histogram is zero between steps: the scan clears what it has read
     LV_CUDA(s, cudaMemsetAsync(B.cell_cnt, 0, 4 * ((size_t)s->grid.base[s->n_types] + 1), s->stream));

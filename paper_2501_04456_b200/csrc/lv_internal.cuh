@@ -52,6 +52,9 @@ struct LvDev {
     int32_t list_cap;        // entries per NP
     float skin;              // list radius = r_c,ab + skin
     float half_skin2;        // rebuild when an NP has moved farther than this (squared) since the build
+    // LV_FORCE_TILE: a target of type a more than this many cells of its grid along x from a
+    // tile's first target starts a new tile
+    int32_t tile_cells[LV_MAX_TYPES];
 };
 
 // Device-resident scalars.
@@ -126,6 +129,11 @@ cudaError_t lvk_pair_force_list(const LvDev &P, const LvBufs &B, cudaStream_t st
 cudaError_t lvk_update_list(const LvDev &P, const LvBufs &B, cudaStream_t st);
 cudaError_t lvk_keys_sorted(const LvDev &P, const LvBufs &B, uint32_t *out, cudaStream_t st);
 cudaError_t lvk_pair_force(const LvDev &P, const LvBufs &B, int variant, cudaStream_t st);
+// shared-candidate-stream kernel (lv_force_tile.cu): `substreams` lanes per target (1 .. 32, a
+// power of two); lvk_tile_prepare raises its shared-memory limit (call once, outside capture)
+cudaError_t lvk_tile_prepare();
+cudaError_t lvk_pair_force_tile(const LvDev &P, const LvBufs &B, int substreams, bool charged, cudaStream_t st);
+bool lvk_any_charge(const LvDev &P);
 // hash_next: also hash + histogram the new positions for the next step's counting sort
 cudaError_t lvk_update(const LvDev &P, const LvBufs &B, bool hash_next, cudaStream_t st);
 cudaError_t lvk_pack_state(const LvDev &P, const LvBufs &B, const float *pos, const float *vel,

@@ -9,6 +9,7 @@
 // A3 (the sort) is in lv_sort.cu.  State layout: float4 pos = (x, y, z, type
 // bits), float4 vel = (vx, vy, vz, id bits), 16-byte aligned SoA.
 #include "lv_internal.cuh"
+#include "lv_device.cuh"
 
 #include <cstring>
 #include <cmath>
@@ -16,23 +17,6 @@
 namespace {
 
 constexpr int kThreads = 128;
-
-// Skin-list steps run the cell rebuild only when the device-side flag of this step is
-// raised (LvDevState::rebuild); `guard` is null on every other path.
-__device__ __forceinline__ bool skipped(const LvDevState *guard)
-{
-    return guard != nullptr && guard->rebuild[guard->step & 1] == 0u;
-}
-
-__device__ __forceinline__ int cell_coord(float x, float lo, float inv_h, int G)
-{
-    // fp32 contract #1: t = fl(fl(x - lo) * inv_h), clamp(floor t), NaN -> 0
-    float t = __fmul_rn(__fsub_rn(x, lo), inv_h);
-    float f = floorf(t);
-    if (!(f >= 0.0f)) return 0;
-    if (f > (float)(G - 1)) return G - 1;
-    return (int)f;
-}
 
 // Pair-interleaved copy of the cell-sorted positions (LvBufs::posP): slot k goes to
 // floats {x, y, z, w} at 8 (k >> 1) + (k & 1) + {0, 2, 4, 6}.  The thread of the last
@@ -293,19 +277,6 @@ k_keys_sorted(int n, const uint32_t *__restrict__ key, const uint32_t *__restric
 }
 
 // ------------------------------------------------------------ A6 pair force
-__device__ __forceinline__ float rcp_approx(float x)
-{
-    float y;
-    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
-    return y;
-}
-__device__ __forceinline__ float rsqrt_approx(float x)
-{
-    float y;
-    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
-    return y;
-}
-
 // One thread per cell-sorted NP.  For every neighbour type b the thread walks
 // the (2 w_ab + 1)^2 rows of grid b around its own cell; a row is ONE contiguous
 // run of sorted slots [off[first cell], off[last cell + 1]).
@@ -376,7 +347,6 @@ k_pair_force(const __grid_constant__ LvDev P, const float4 *__restrict__ pos,
 constexpr int kFThreads = 128;
 constexpr int kQCap = 16;       // queue slots per thread (8 KB per block: leaves the L1 its room)
 constexpr int kChunk = 4;       // candidates per lane and iteration
-constexpr unsigned kFull = 0xffffffffu;
 
 // pos[.] if `take`, else (+inf, ?, ?, ?); one predicated LDG, no branch
 __device__ __forceinline__ float4 ld_pos_if(const float4 *p, bool take)
@@ -543,40 +513,6 @@ constexpr int kSThreads = LV_S_THREADS;
 constexpr int kSegCap = LV_S_SEGCAP;       // segments per lane between walks
 constexpr int kSChunk = LV_S_CHUNK;
 
-template <int N> struct IntC { static constexpr int value = N; };
-
-// Two fp32 lanes in one 64-bit register pair (sm_100 FADD2 / FMUL2 / FFMA2): each half is
-// an IEEE round-to-nearest operation, so contract #2 holds per half; one instruction issue
-// serves two candidates.
-typedef unsigned long long f32x2;
-__device__ __forceinline__ f32x2 pack2(float lo, float hi)
-{
-    f32x2 r;
-    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
-    return r;
-}
-__device__ __forceinline__ void unpack2(f32x2 v, float &lo, float &hi)
-{
-    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
-}
-__device__ __forceinline__ f32x2 sub2(f32x2 a, f32x2 b)
-{
-    f32x2 r;
-    asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
-    return r;
-}
-__device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b)
-{
-    f32x2 r;
-    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
-    return r;
-}
-__device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c)
-{
-    f32x2 r;
-    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
-    return r;
-}
 
 // kMode 0: forces, scalar walk.  1: forces, packed walk.  2: no forces -- the same row and
 // walk phases with the cut-off widened by the skin EMIT the in-range slots into the lane's
@@ -1567,7 +1503,7 @@ cudaError_t lvk_bounds_scatter(const LvDev &P, const LvBufs &B, bool packed, cud
     return cudaGetLastError();
 }
 
-static bool any_charge(const LvDev &P)
+bool lvk_any_charge(const LvDev &P)
 {
     bool charged = false;
     for (int a = 0; a < P.n_types; ++a)
@@ -1583,7 +1519,7 @@ cudaError_t lvk_pair_force(const LvDev &P, const LvBufs &B, int variant, cudaStr
         k_pair_force_q<<<(P.n + kFThreads - 1) / kFThreads, kFThreads, 0, st>>>(P, B.posB, B.cell_off,
                                                                              B.force);
     else {
-        const bool charged = any_charge(P);
+        const bool charged = lvk_any_charge(P);
         const int blocks = (P.n + kSThreads - 1) / kSThreads;
         if (variant == 3) {
             if (charged)
@@ -1616,7 +1552,7 @@ cudaError_t lvk_list_build(const LvDev &P, const LvBufs &B, cudaStream_t st)
 cudaError_t lvk_pair_force_list(const LvDev &P, const LvBufs &B, cudaStream_t st)
 {
     const int blocks = (P.n + kSThreads - 1) / kSThreads;
-    if (any_charge(P))
+    if (lvk_any_charge(P))
         k_pair_force_list<true><<<blocks, kSThreads, 0, st>>>(P, B.posA, B.posB, B.list, B.list_rows,
                                                               B.force, B.st);
     else

@@ -544,8 +544,9 @@ def test_explicit_interaction_matrix(B, orc):
     sim.close()
 
 
-VARIANTS = [  # (sort, force kernel): lv_set_option; (0, 2) is the default path
-    (1, 0), (1, 1), (1, 2), (0, 0), (0, 1), (0, 3), (1, 3),
+VARIANTS = [  # (sort, force kernel, tile sub-streams): lv_set_option; (0, 2) is the default path
+    (1, 0, None), (1, 1, None), (1, 2, None), (0, 0, None), (0, 1, None), (0, 3, None), (1, 3, None),
+    (0, 4, 1), (0, 4, 2), (0, 4, 4), (1, 4, 8), (0, 4, 16), (0, 4, 32),
 ]
 
 
@@ -568,9 +569,11 @@ def test_implementation_options_do_not_change_results(B, orc, name, n, cpc):
     x0, v0, _, _, _ = ref.get_state()
     ids0 = ref.get_debug(B.DBG_IDS_SORTED)
     ref.close()
-    for sort, fk in VARIANTS:
-        sim = B.Simulation.from_workload(w, cells_per_cut=cpc,
-                                         options={B.OPT_SORT: sort, B.OPT_FORCE_KERNEL: fk})
+    for sort, fk, sub in VARIANTS:
+        opts = {B.OPT_SORT: sort, B.OPT_FORCE_KERNEL: fk}
+        if sub is not None:
+            opts[B.OPT_TILE_SUBSTREAMS] = sub
+        sim = B.Simulation.from_workload(w, cells_per_cut=cpc, options=opts)
         sim.compute_forces()
         assert np.array_equal(sim.get_debug(B.DBG_KEYS), key)
         assert np.array_equal(sim.get_debug(B.DBG_KEYS_SORTED), ks)
