@@ -282,7 +282,8 @@ typedef struct {
     uint32_t background, droplet;
 } lv_view;
 
-/* zbuf_dev: DEVICE scratch of width*height*8 bytes, 8-byte aligned, owned by the caller,
+/* zbuf_dev: DEVICE scratch of width*height*8 bytes (width*height*12 when rgba is host memory:
+ * the image is staged behind the depth keys), 8-byte aligned, owned by the caller,
  * clobbered.  rgba: width*height uint32, written; host or device per on_device.
  * Synchronises when rgba is host memory; the state does not change. */
 int lv_render(lv_sim *s, const lv_view *view, void *zbuf_dev, uint32_t *rgba, int on_device);
@@ -302,8 +303,9 @@ int lv_render(lv_sim *s, const lv_view *view, void *zbuf_dev, uint32_t *rgba, in
  * fp32 NP radius);
  * among several the smallest (bits(d2) << 32 | palette[type]) wins; a pixel no NP marks
  * shows `droplet`.  Pixels are 0xAABBGGRR with AA = 0xff.
- * scratch_dev: DEVICE scratch of width*height*8 + (width + height)*8 bytes, 8-byte aligned,
- * owned by the caller, clobbered.  rgba: width*height uint32, host or device per on_device.
+ * scratch_dev: DEVICE scratch of width*height*8 + (width + height)*8 bytes (+ width*height*4
+ * when rgba is host memory: the image is staged there), 8-byte aligned, owned by the caller,
+ * clobbered.  rgba: width*height uint32, host or device per on_device.
  * Synchronises; the state does not change. */
 typedef struct {
     int32_t width, height;               /* 1..8192 each */
@@ -349,9 +351,10 @@ int lv_stage_timing(lv_sim *s, int capacity);
 int lv_read_stage_timing(lv_sim *s, double *ms_stage_sum, double *ms_step_sum, int64_t *steps);
 
 /* Measurement aid: FP32 FMA throughput of this GPU from a register-resident
- * independent-FMA kernel on `cuda_stream`; writes TFLOP/s (host).  The
- * denominator of the pair-force kernel's ALU roofline. */
-int lv_measure_fp32_peak(void *cuda_stream, double *tflops);
+ * independent-FMA kernel on `cuda_stream`; writes TFLOP/s (host).  scratch_dev: DEVICE
+ * scratch of >= 256 bytes owned by the caller.  The denominator of the pair-force kernel's
+ * ALU roofline. */
+int lv_measure_fp32_peak(void *cuda_stream, void *scratch_dev, double *tflops);
 
 int lv_destroy(lv_sim *s);
 const char *lv_strerror(int code);

@@ -110,7 +110,7 @@ def load():
     L.lv_step_profiled.argtypes = [vp, C.POINTER(C.c_float)]
     L.lv_stage_timing.argtypes = [vp, C.c_int]
     L.lv_read_stage_timing.argtypes = [vp, dp, dp, C.POINTER(C.c_int64)]
-    L.lv_measure_fp32_peak.argtypes = [vp, dp]
+    L.lv_measure_fp32_peak.argtypes = [vp, vp, dp]
     L.lv_destroy.argtypes = [vp]
     L.lv_strerror.argtypes = [C.c_int]
     L.lv_strerror.restype = C.c_char_p
@@ -322,7 +322,10 @@ class Simulation:
             v.palette[a] = int(c)
         v.background, v.droplet = int(background), int(droplet)
         with torch.cuda.device(self.device):
-            zbuf = torch.empty(int(width) * int(height), dtype=torch.int64, device=self.device)
+            n_px = int(width) * int(height)
+            # depth keys (8 B per pixel) + the staged image for host output (4 B per pixel)
+            zbuf = torch.empty(n_px + (0 if on_device else (n_px + 1) // 2), dtype=torch.int64,
+                               device=self.device)
             zbuf.record_stream(self.stream)
             if on_device:
                 img = torch.empty((int(height), int(width)), dtype=torch.int32, device=self.device)
@@ -346,7 +349,8 @@ class Simulation:
         m.droplet = int(droplet)
         w_, h_ = max(int(width), 0), max(int(height), 0)
         with torch.cuda.device(self.device):
-            scratch = torch.empty(w_ * h_ + w_ + h_ + 1, dtype=torch.int64, device=self.device)
+            scratch = torch.empty(w_ * h_ + w_ + h_ + 1 + (0 if on_device else (w_ * h_ + 1) // 2),
+                                  dtype=torch.int64, device=self.device)
             scratch.record_stream(self.stream)
             if on_device:
                 img = torch.empty((h_, w_), dtype=torch.int32, device=self.device)
@@ -402,9 +406,13 @@ class Simulation:
         return dict(zip(self.STAGES, [float(v) for v in st])), tot.value, int(n.value)
 
     def measure_fp32_peak(self) -> float:
+        import torch
         t = C.c_double()
-        self._check(self.L.lv_measure_fp32_peak(self.stream.cuda_stream, C.byref(t)),
+        with torch.cuda.device(self.device):
+            scratch = torch.empty(256, dtype=torch.uint8, device=self.device)
+        self._check(self.L.lv_measure_fp32_peak(self.stream.cuda_stream, scratch.data_ptr(), C.byref(t)),
                     "lv_measure_fp32_peak")
+        self.stream.synchronize()
         return t.value
 
     def synchronize(self):

@@ -101,6 +101,9 @@ int derive_grid(lv_sim *s)
         for (int b = 0; b < T; ++b) {
             const double w = std::ceil(s->rcut[a * LV_MAX_TYPES + b] * (1.0 + 1.0 / 1024.0) / g.h[b]);
             if (w > 100.0) return LV_E_ARG;
+            // the stencil of the skin list (r_c,ab + skin) is kept in an int8 as well
+            if (std::ceil((s->rcut[a * LV_MAX_TYPES + b] + s->skin) * (1.0 + 1.0 / 1024.0) / g.h[b]) > 100.0)
+                return LV_E_ARG;
             g.w[a * LV_MAX_TYPES + b] = (int32_t)w;
         }
     int bits = 1;
@@ -319,13 +322,13 @@ int build_graph(lv_sim *s)
     s->hashed = false;
     cudaGraph_t g = nullptr;
     cudaError_t e = cudaStreamEndCapture(s->stream, &g);
-    if (rc != LV_OK) { if (g) cudaGraphDestroy(g); return rc; }
+    if (rc != LV_OK) { if (g) cudaGraphDestroy(g); return rc; }     // the capture has been ended above
     if (e != cudaSuccess) return cuda_fail(s, e, "cudaStreamEndCapture");
     s->graph = g;
     size_t nn = 0;
     LV_CUDA(s, cudaGraphGetNodes(g, nullptr, &nn));
     cudaGraphNode_t *nodes = (cudaGraphNode_t *)malloc(sizeof(cudaGraphNode_t) * (nn ? nn : 1));
-    if (!nodes) return LV_E_NOMEM;
+    if (!nodes) { cudaGraphDestroy(g); s->graph = nullptr; return LV_E_NOMEM; }
     cudaError_t e2 = cudaGraphGetNodes(g, nodes, &nn);
     int kernels = 0;
     for (size_t i = 0; e2 == cudaSuccess && i < nn; ++i) {
@@ -333,9 +336,14 @@ int build_graph(lv_sim *s)
         if (cudaGraphNodeGetType(nodes[i], &t) == cudaSuccess && t == cudaGraphNodeTypeKernel) ++kernels;
     }
     free(nodes);
-    if (e2 != cudaSuccess) return cuda_fail(s, e2, "cudaGraphGetNodes");
+    if (e2 == cudaSuccess) e2 = cudaGraphInstantiate(&s->graph_exec, g, 0);
+    if (e2 != cudaSuccess) {          // leave no half-built graph behind
+        cudaGraphDestroy(g);
+        s->graph = nullptr;
+        s->graph_exec = nullptr;
+        return cuda_fail(s, e2, "cudaGraphGetNodes / cudaGraphInstantiate");
+    }
     s->launches_per_step = kernels;
-    LV_CUDA(s, cudaGraphInstantiate(&s->graph_exec, g, 0));
     return LV_OK;
 }
 
@@ -636,13 +644,14 @@ int lv_observe_rdf(lv_sim *s, double dr, int n_bins, uint64_t *hist, double *g)
     if (!s->bound || !s->state_set) return LV_E_ORDER;
     if (hist) memset(hist, 0, 8 * (size_t)n_bins);
     if (g) for (int k = 0; k < n_bins; ++k) g[k] = 0.0;
+    for (int b = 0; b < s->n_types; ++b)       // the pair walk keeps its stencil half-width in an int8
+        if (std::ceil(dr * (double)n_bins * (1.0 + 1.0 / 1024.0) / s->grid.h[b]) > 100.0) return LV_E_ARG;
     if (s->n == 0) return LV_OK;
     // cell structures of the current state (steps (i) of PAPER.md:64), then the pair walk
     for (int k = 0; k < 3; ++k) {
         int rc = enqueue_stage(s, k);
         if (rc != LV_OK) return rc;
     }
-    s->force_order_b = true;
     unsigned long long *dh = nullptr;
     double *ds = nullptr;
     int rc = obs_scratch(s, n_bins, &dh, &ds);
@@ -737,7 +746,6 @@ int lv_observe_clusters(lv_sim *s, double bond_factor, int32_t *labels, int64_t 
         int rc = enqueue_stage(s, k);
         if (rc != LV_OK) return rc;
     }
-    s->force_order_b = true;
     // scratch in the staging area: 3 uint32[n] | int32 labels[n] | 34 u64 statistics
     const size_t n = (size_t)s->n;
     if ((28 * n > 65600 ? 28 * n : 65600) < 16 * n + 34 * 8 + 8) return LV_E_ARG;   // staging >= 65600 B
@@ -774,18 +782,11 @@ int lv_render(lv_sim *s, const lv_view *view, void *zbuf_dev, uint32_t *rgba, in
     LV_CUDA(s, cudaStreamSynchronize(s->stream));
     const double R = lv_radius_of(s->sched_mode, s->R0, s->R1, s->sched_steps, st.step);
     const size_t n_px = (size_t)view->width * view->height;
-    uint32_t *drgba = rgba;
-    if (!on_device) {
-        // the image is staged behind the depth keys would need more scratch: use the tail of zbuf?
-        // no -- keep it simple: a temporary device image
-        LV_CUDA(s, cudaMallocAsync((void **)&drgba, 4 * n_px, s->stream));
-    }
+    // host output: the image is staged in the caller's scratch, behind the depth keys
+    uint32_t *drgba = on_device ? rgba : (uint32_t *)((unsigned long long *)zbuf_dev + n_px);
     cudaError_t e = lvk_render(s->dev, s->bufs, view, rot, R, (unsigned long long *)zbuf_dev, drgba, s->stream);
-    if (e == cudaSuccess && !on_device)
+    if (e == cudaSuccess && !on_device) {
         e = cudaMemcpyAsync(rgba, drgba, 4 * n_px, cudaMemcpyDeviceToHost, s->stream);
-    if (!on_device) {
-        cudaError_t e2 = cudaFreeAsync(drgba, s->stream);
-        if (e == cudaSuccess) e = e2;
         if (e == cudaSuccess) e = cudaStreamSynchronize(s->stream);
     }
     if (e != cudaSuccess) return cuda_fail(s, e, "lv_render");
@@ -825,15 +826,11 @@ int lv_render_surface(lv_sim *s, const lv_surface_map *map, void *scratch_dev, u
     unsigned long long *zbuf = (unsigned long long *)scratch_dev;
     float *tab_dev = (float *)(zbuf + n_px);
     LV_CUDA(s, cudaMemcpyAsync(tab_dev, tab, 4 * (2 * (size_t)W + 2 * (size_t)H), cudaMemcpyHostToDevice, s->stream));
-    uint32_t *drgba = rgba;
-    if (!on_device) LV_CUDA(s, cudaMallocAsync((void **)&drgba, 4 * n_px, s->stream));
+    // host output: the image is staged in the caller's scratch, behind the keys and the tables
+    uint32_t *drgba = on_device ? rgba : (uint32_t *)(tab_dev + 2 * ((size_t)W + (size_t)H));
     cudaError_t e = lvk_render_surface(s->dev, s->bufs, map, R, tab_dev, zbuf, drgba, s->stream);
     if (e == cudaSuccess && !on_device)
         e = cudaMemcpyAsync(rgba, drgba, 4 * n_px, cudaMemcpyDeviceToHost, s->stream);
-    if (!on_device) {
-        cudaError_t e2 = cudaFreeAsync(drgba, s->stream);
-        if (e == cudaSuccess) e = e2;
-    }
     // synchronise in both modes: `tab` is pageable host memory read by the stream
     if (e == cudaSuccess) e = cudaStreamSynchronize(s->stream);
     if (e != cudaSuccess) return cuda_fail(s, e, "lv_render_surface");
@@ -1012,15 +1009,14 @@ int lv_read_stage_timing(lv_sim *s, double *ms_stage_sum, double *ms_step_sum, i
     return LV_OK;
 }
 
-int lv_measure_fp32_peak(void *cuda_stream, double *tflops)
+int lv_measure_fp32_peak(void *cuda_stream, void *scratch_dev, double *tflops)
 {
-    if (!tflops) return LV_E_ARG;
+    if (!tflops || !scratch_dev) return LV_E_ARG;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     int dev = 0, sms = 0;
     if (cudaGetDevice(&dev) != cudaSuccess) return LV_E_CUDA;
     if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return LV_E_CUDA;
-    float *scratch = nullptr;
-    if (cudaMalloc(&scratch, 256) != cudaSuccess) return LV_E_CUDA;   // measurement aid only
+    float *scratch = (float *)scratch_dev;
     cudaEvent_t e0, e1;
     cudaEventCreate(&e0);
     cudaEventCreate(&e1);
@@ -1037,7 +1033,6 @@ int lv_measure_fp32_peak(void *cuda_stream, double *tflops)
     }
     cudaEventDestroy(e0);
     cudaEventDestroy(e1);
-    cudaFree(scratch);
     if (e != cudaSuccess) return LV_E_CUDA;
     *tflops = best;
     return LV_OK;

@@ -741,8 +741,10 @@ k_pair_force_s(const __grid_constant__ LvDev P, const float4 *__restrict__ pos,
         auto bounds = [&](int y, int z, float rem, uint32_t &js, uint32_t &je) {
             const float remp = fmaxf(rem, 1e-6f);
             const float xh = fmaf(remp, rsqrt_approx(remp), marg);   // sqrt to 2 ulp, inside marg
-            const int xa = max(xlo, __float2int_rd(tx - xh));
-            const int xb = min(xhi, __float2int_rd(tx + xh));
+            // cells 0 and G - 1 are open outwards (contract #1 clamps): a target beyond the grid
+            // still sees the border cell its neighbours were clamped into
+            const int xa = max(xlo, min(__float2int_rd(tx - xh), g.G - 1));
+            const int xb = min(xhi, max(__float2int_rd(tx + xh), 0));
             const bool ok = rem > 1e-6f && xa <= xb;
             const uint32_t r0 = g.base + (uint32_t)((z * g.G + y) * g.G);
             js = __ldg(off + (ok ? r0 + xa : own));
@@ -931,17 +933,27 @@ k_update(const __grid_constant__ LvDev P, const float4 *__restrict__ posB_,
         if (i < (int)P.n_scan_tiles) scan_tile[i] = 0ull;   // re-arm the next step's scan
         if (i == 0) *scan_ticket = 0u;
     }
-    const long long n = st->step;                      // index of this step
-    const bool rebuilt = kList ? st->rebuild[n & 1] != 0u : true;
+    // thread 0 alone reads the step index and this step's rebuild flag and hands them to the
+    // block through shared memory; its loads are fenced before it takes the ticket, so the
+    // block that takes the last ticket (and overwrites both) has seen every block's reads
     __shared__ double s_R;                             // (iii), R9: once per block, fp64
-    if (threadIdx.x == 0) s_R = lv_radius_of(P.sched_mode, P.R0, P.R1, P.sched_steps, n + 1);
-    __syncthreads();
-    // the block that takes the last ticket has seen every block read `step`
-    if (threadIdx.x == 0 && atomicAdd(&st->ticket, 1u) == gridDim.x - 1) {
-        st->ticket = 0u;
-        st->step = n + 1;
-        if (kList) st->rebuild[n & 1] = 0u;            // ... and this step's rebuild flag
+    __shared__ long long s_n;
+    __shared__ unsigned int s_rebuilt;
+    if (threadIdx.x == 0) {
+        const long long n0 = st->step;                 // index of this step
+        s_n = n0;
+        s_rebuilt = kList ? st->rebuild[n0 & 1] : 1u;
+        s_R = lv_radius_of(P.sched_mode, P.R0, P.R1, P.sched_steps, n0 + 1);
+        __threadfence();
+        if (atomicAdd(&st->ticket, 1u) == gridDim.x - 1) {
+            st->ticket = 0u;
+            st->step = n0 + 1;
+            if (kList) st->rebuild[n0 & 1] = 0u;       // ... and this step's rebuild flag
+        }
     }
+    __syncthreads();
+    const long long n = s_n;
+    const bool rebuilt = s_rebuilt != 0u;
     if (i >= P.n) return;
     const float4 *posB = rebuilt ? posB_ : posA;
     const float4 *velB = rebuilt ? velB_ : velA;

@@ -185,19 +185,157 @@ def test_one_step_moving_interface_near_wall(B, orc):
     sim.close()
 
 
-@pytest.mark.parametrize("name,n", [("C1", None), ("C2", 8192), ("C4", 8000), ("T8", 6000)])
-def test_hundred_steps(B, orc, name, n):
+@pytest.mark.parametrize("name,n,cpc", [("C1", None, None), ("C2", 8192, None), ("C4", 8000, None),
+                                        ("T8", 6000, None), ("C3", 20000, [1, 2, 2]), ("C5", 20001, None),
+                                        ("C3", None, "tuned")])
+def test_hundred_steps(B, orc, name, n, cpc):
+    """100 steps on the DEFAULT path (north_star: "states after 100 steps within 1e-3 of the
+    droplet radius"), C3 -- the bench workload -- also at full size with its tuned grids."""
     w = workload(name, n)
+    if cpc == "tuned":
+        cpc = w.tuned_cells_per_cut
     p = orc.params_from_workload(w)
     xo, vo, bad = orc.step(p, w.pos, w.vel, w.type, step0=0, nsteps=100)
-    sim = B.Simulation.from_workload(w)
+    sim = B.Simulation.from_workload(w, cells_per_cut=cpc)
     sim.step(100)
     xg, vg, _, R, st = sim.get_state()
     assert bad == 0 and st == 100
     assert R == pytest.approx(orc.radius(p, 100), rel=1e-15)
     d = np.linalg.norm(xg.astype(np.float64) - xo, axis=1)
     assert d.max() <= 1e-3 * R, d.max() / R
+    assert sim.status() == 0
     sim.close()
+
+
+def test_forces_at_the_benched_snapshots(B, orc):
+    """The later states bench.py times (C3, N = 2.5e5, tuned grids, steps 10 000 and 17 000 of
+    the shrinking schedule: ~210 and ~580 in-range neighbours per NP): the GPU's own state at
+    those steps goes to both sides; neighbour counts bit-exact, forces to 1e-5 S, with the
+    default kernel and with the shared-candidate-stream kernel."""
+    w = workload("C3", None)
+    p = orc.params_from_workload(w)
+    cpc = w.tuned_cells_per_cut
+    sim = B.Simulation.from_workload(w, cells_per_cut=cpc)
+    tile = B.Simulation.from_workload(w, cells_per_cut=cpc, load_state=False,
+                                      options={B.OPT_FORCE_KERNEL: B.FORCE_TILE, B.OPT_TILE_SUBSTREAMS: 8})
+    cur = 0
+    for target, lo in ((10000, 150), (17000, 400)):
+        sim.step(target - cur)
+        cur = target
+        x, v, t, R, st = sim.get_state()
+        assert st == target and sim.status() == 0
+        Fo, So, co, _ = orc.pair_forces(p, x, t, "cells")
+        assert co.mean() > lo
+        sim.compute_forces()
+        Fg, cg = sim.get_forces()
+        assert np.array_equal(cg, co)
+        assert force_error(Fg, Fo, So) <= FORCE_TOL
+        tile.set_state(x, v, t, st)
+        tile.compute_forces()
+        Ft, ct = tile.get_forces()
+        assert np.array_equal(ct, co)
+        assert force_error(Ft, Fo, So) <= FORCE_TOL
+    sim.close(); tile.close()
+
+
+@pytest.mark.parametrize("name,n,cpc", [("C2", 8192, [2, 2]), ("C3", 20000, [1, 2, 2]), ("C4", 8000, None)])
+def test_steady_state_permutation_against_the_oracle(B, orc, name, n, cpc):
+    """fp32 contract #3 in steady state (hash fused into the update kernel, CUDA-graph replay):
+    the slot order of step k + 1 must be the STABLE sort, by the oracle's cell keys of the
+    positions after step k, of the slot order of step k."""
+    w = workload(name, n)
+    p = orc.params_from_workload(w)
+    g = orc.grid_spec(p, cpc)
+    sim = B.Simulation.from_workload(w, cells_per_cut=cpc)
+    sim.step(5)
+    ids_prev = sim.get_debug(B.DBG_IDS_SORTED).astype(np.int64)
+    moved = 0
+    for k in range(20):
+        x, v, t, R, st = sim.get_state()              # state the next step starts from, by id
+        key, ks, perm, off = orc.cell_structures(g, x[ids_prev], t[ids_prev])
+        sim.step(1)
+        ids_next = sim.get_debug(B.DBG_IDS_SORTED).astype(np.int64)
+        assert np.array_equal(ids_next, ids_prev[perm.astype(np.int64)])
+        moved += int((ids_next != ids_prev).sum())
+        ids_prev = ids_next
+    assert moved > 0                                   # NPs did change cells meanwhile
+    sim.close()
+
+
+def test_one_step_late_schedule_near_wall(B, orc):
+    """Late in the schedule many NPs are pressed against the moving interface: the GPU runs
+    C3@20000 to step 6 000, that state goes to both sides, one step to the one-step bars (the
+    wall term in the force scale)."""
+    w = workload("C3", 20000)
+    p = orc.params_from_workload(w)
+    run = B.Simulation.from_workload(w, cells_per_cut=[1, 2, 2])
+    run.step(6000)
+    x, v, t, R, st = run.get_state()
+    assert st == 6000 and run.status() == 0
+    run.close()
+    xo, vo, bad, Fp, Fe = orc.step(p, x, v, t, step0=st, nsteps=1, want_forces=True)
+    assert bad == 0
+    assert (np.abs(Fe).max(axis=1) > 1.0).sum() > 300         # the wall is really felt
+    _, So, _, _ = orc.pair_forces(p, x, t, "cells")
+    Sw = np.abs(Fe).sum(axis=1)
+    sim = B.Simulation.from_workload(w, load_state=False)
+    sim.set_state(x, v, t, st)
+    sim.step(1)
+    xg, vg, _, Rg, st1 = sim.get_state()
+    assert st1 == st + 1 and Rg == pytest.approx(orc.radius(p, st + 1), rel=1e-15)
+    vel_pos_check(w, p, xo, vo, xg, vg, So + Sw, Rg)
+    sim.close()
+
+
+def test_forces_survive_an_observe_call(B):
+    """lv_get_forces after lv_step + lv_observe_*: the observables re-sort the B copy, the
+    forces of the last step must still be attributed to the right NPs."""
+    w = workload("C2", 8192)
+    sim = B.Simulation.from_workload(w)
+    sim.step(25)
+    F0, c0 = sim.get_forces()
+    sim.observe_rdf(0.05, 100)
+    F1, c1 = sim.get_forces()
+    sim.observe_clusters(1.5)
+    F2, c2 = sim.get_forces()
+    assert np.array_equal(F0, F1) and np.array_equal(c0, c1)
+    assert np.array_equal(F0, F2) and np.array_equal(c0, c2)
+    assert c0.sum() > 0
+    sim.close()
+
+
+@pytest.mark.parametrize("fk,sub", [(0, None), (1, None), (2, None), (3, None), (4, 1), (4, 8)])
+def test_bonded_pair_outside_the_grid(B, orc, fk, sub):
+    """NPs beyond the grid are clamped into the border cells (R22, warning only): two bonded
+    NPs outside along +x, two along -x and two along +y must still see each other, in every
+    force kernel and through the neighbour list."""
+    w = W.make_workload("C1", None)
+    p = orc.params_from_workload(w)
+    pos = w.pos.copy()
+    far = 40.0                                   # grid half-width ~ 22.5
+    pos[0] = [far, 0.3, 0.2];  pos[1] = [far + 1.1, 0.3, 0.2]
+    pos[2] = [-far, -0.4, 0.1]; pos[3] = [-far - 1.05, -0.4, 0.1]
+    pos[4] = [0.5, far, 0.0];  pos[5] = [0.5, far + 1.2, 0.0]
+    Fo, So, co, _ = orc.pair_forces(p, pos, w.type, "brute")
+    assert np.all(co[:6] == 1)
+    opts = {B.OPT_FORCE_KERNEL: fk}
+    if sub is not None:
+        opts[B.OPT_TILE_SUBSTREAMS] = sub
+    sim = B.Simulation.from_workload(w, load_state=False, options=opts)
+    sim.set_state(pos, w.vel, w.type, 0)
+    sim.compute_forces()
+    Fg, cg = sim.get_forces()
+    assert sim.status() == B.ST_OUTSIDE_GRID
+    assert np.array_equal(cg, co)
+    assert force_error(Fg, Fo, So) <= FORCE_TOL
+    sim.close()
+    if fk == 2:
+        lst = B.Simulation.from_workload(w, load_state=False, neighbour_list=(0.3, 64))
+        lst.set_state(pos, np.zeros_like(w.vel), w.type, 0)
+        lst.step(1)
+        Fl, cl = lst.get_forces()
+        assert np.array_equal(cl, co)
+        lst.close()
 
 
 @pytest.mark.parametrize("mode", ["LINEAR", "R2LAW"])
