@@ -47,7 +47,7 @@ extern "C" {
 #define LV_E_CUDA       -4   /* a CUDA runtime call failed; see lv_last_cuda_error */
 #define LV_E_NONFINITE  -5   /* sticky: a non-finite position or velocity appeared (R6) */
 #define LV_E_NOMEM      -6   /* host allocation failed */
-#define LV_E_CAPACITY   -7   /* sticky: the skin neighbour list overflowed (LV_ST_LIST_OVERFLOW) */
+#define LV_E_CAPACITY   -7   /* reserved (was: skin list overflow; now a warning, LV_ST_LIST_OVERFLOW) */
 
 /* droplet schedule modes: step (iii); radius-square law PAPER.md:58 */
 #define LV_SCHED_CONST   0
@@ -61,7 +61,7 @@ extern "C" {
 /* status bits (lv_get_status); warnings do not stop the simulation */
 #define LV_ST_NONFINITE    1u   /* error: also returned as LV_E_NONFINITE */
 #define LV_ST_OUTSIDE_GRID 2u   /* warning: an NP was clamped into a border cell (R22) */
-#define LV_ST_LIST_OVERFLOW 4u  /* error: an NP has more neighbours than the list capacity */
+#define LV_ST_LIST_OVERFLOW 4u  /* warning: the skin list did not fit its pool; those steps used the cells */
 #define LV_ST_BAD_TYPE     8u   /* error: lv_set_state saw a type outside [0, n_types); that NP was
                                    loaded as type 0 and lv_get_state returns LV_E_ARG */
 
@@ -174,23 +174,35 @@ int lv_set_grid(lv_sim *s, const int32_t *cells_per_cut);
 #define LV_OPT_TILE_SPAN       4
 int lv_set_option(lv_sim *s, int option, int value);
 
-/* Optional throughput variant: a persistent "skin" neighbour
- * list.  The paper rebuilds the cells every step only "to identify which [NPs] are close
- * to each other and can interact"; with capacity > 0 lv_step keeps, per NP,
- * the slots of every NP within r_c,ab + skin at the last rebuild, evaluates the pair force
- * from that list (same fp32 contract #2, so the neighbour counts stay bit-identical and
- * the forces agree to rounding), and rebuilds cells + list on the device -- no host
- * round trip -- at the first step after any NP has moved farther than skin/2 from where it
- * was at the build.  skin: length units, > 0.  capacity: list entries per NP (the
- * workspace grows by 4 * capacity bytes per NP); if an NP has more neighbours the sticky
- * LV_ST_LIST_OVERFLOW is set and lv_get_state returns LV_E_CAPACITY.  capacity = 0
- * (default) switches the variant off: every step rebuilds, as the paper does.  Needs
- * LV_SORT_COUNTING.  lv_compute_forces always uses the cells. */
+/* Persistent "skin" neighbour list.  The paper rebuilds the cells
+ * every step only "to identify which [NPs] are close to each other and can interact"
+ * (PAPER.md:64); with capacity != 0 lv_step keeps, per NP, the slots of every NP within
+ * r_c,ab + skin at the last rebuild, evaluates the pair force from that list (same fp32
+ * contract #2, so the neighbour counts stay bit-identical and the forces agree to rounding),
+ * and rebuilds cells + list on the device -- no host round trip -- at the first step after any
+ * NP has moved farther than skin/2 from where it was at the build.
+ *   skin      length units; <= 0: automatic, a tenth of the smallest cut-off (needs lv_set_types
+ *             first).
+ *   capacity  > 0: the list pool holds capacity entries per NP ON AVERAGE (4 * capacity bytes per
+ *             NP of workspace; a crowded NP may use more than its share); -1: automatic, 1024
+ *             entries per NP but at most 2 GiB; 0 (default): the variant is off and every step
+ *             rebuilds the cells, as the paper does.
+ * The list is built in two passes (count, then fill) into per-warp tiles whose height is the
+ * longest list of the warp.  If a rebuild would need more than the pool, nothing is lost: the
+ * warning bit LV_ST_LIST_OVERFLOW is raised and the steps run on the cell kernel (rebuilding the
+ * cells every step) until a later count -- taken every 64th step -- fits again.  The choice
+ * depends only on the state and the step index, so lv_step(a); lv_step(b) == lv_step(a + b)
+ * still holds.  Needs LV_SORT_COUNTING.  lv_compute_forces always uses the cells. */
 int lv_set_neighbour_list(lv_sim *s, double skin, int capacity);
 
 /* Cell/list rebuilds since lv_set_state (host int64, written); counts only steps taken
  * with the neighbour list on.  Synchronises. */
 int lv_get_rebuild_count(lv_sim *s, int64_t *rebuilds);
+
+/* out4 (host int64[4], written): rebuilds since lv_set_state, list entries (padded tiles) the
+ * last count needed, steps taken on the cell kernel because the list did not fit, pool size
+ * in entries.  Synchronises. */
+int lv_get_list_stats(lv_sim *s, int64_t *out4);
 
 /* Bytes of device workspace lv_bind needs (0 if types are not set). */
 size_t lv_workspace_bytes(const lv_sim *s);

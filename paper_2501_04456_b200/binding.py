@@ -30,7 +30,7 @@ FORCE_SIMPLE, FORCE_QUEUED, FORCE_SEGMENTS, FORCE_PACKED, FORCE_TILE = 0, 1, 2, 
 # every symbol include/lv.h declares (tests check the library exports them all)
 SYMBOLS = ["lv_langevin_coeffs", "lv_create", "lv_set_types", "lv_set_forces",
            "lv_set_droplet_schedule", "lv_set_grid", "lv_set_option", "lv_set_neighbour_list",
-           "lv_get_rebuild_count", "lv_observe_rdf", "lv_observe_radial", "lv_observe_clusters", "lv_render", "lv_render_surface", "lv_workspace_bytes", "lv_bind",
+           "lv_get_rebuild_count", "lv_get_list_stats", "lv_observe_rdf", "lv_observe_radial", "lv_observe_clusters", "lv_render", "lv_render_surface", "lv_workspace_bytes", "lv_bind",
            "lv_set_state", "lv_step", "lv_compute_forces", "lv_get_state", "lv_get_forces",
            "lv_get_status", "lv_get_debug", "lv_launches_per_step", "lv_step_profiled",
            "lv_stage_timing", "lv_read_stage_timing",
@@ -89,6 +89,7 @@ def load():
     L.lv_set_option.argtypes = [vp, C.c_int, C.c_int]
     L.lv_set_neighbour_list.argtypes = [vp, C.c_double, C.c_int]
     L.lv_get_rebuild_count.argtypes = [vp, C.POINTER(C.c_int64)]
+    L.lv_get_list_stats.argtypes = [vp, C.POINTER(C.c_int64)]
     L.lv_observe_rdf.argtypes = [vp, C.c_double, C.c_int, C.POINTER(C.c_uint64), dp]
     L.lv_observe_clusters.argtypes = [vp, C.c_double, ip, C.POINTER(C.c_int64), dp,
                                       C.POINTER(C.c_int64), C.POINTER(C.c_uint64)]
@@ -192,6 +193,11 @@ class Simulation:
         r = C.c_int64()
         self._check(self.L.lv_get_rebuild_count(self.h, C.byref(r)), "lv_get_rebuild_count")
         return int(r.value)
+
+    def list_stats(self) -> dict:
+        o = (C.c_int64 * 4)()
+        self._check(self.L.lv_get_list_stats(self.h, o), "lv_get_list_stats")
+        return dict(rebuilds=int(o[0]), entries_used=int(o[1]), fallback_steps=int(o[2]), pool_entries=int(o[3]))
 
     def workspace_bytes(self) -> int:
         return int(self.L.lv_workspace_bytes(self.h))

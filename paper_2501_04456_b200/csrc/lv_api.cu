@@ -20,7 +20,8 @@ struct lv_sim {
     bool hashed = false;
     // skin neighbour list (lv_set_neighbour_list); list_cap = 0: off
     double skin = 0.0;
-    int list_cap = 0;
+    int list_cap = 0;               // 0: off; > 0: pool of list_cap entries per NP; -1: automatic pool
+    size_t list_pool_rows = 0;      // pool in rows of 32 entries (derived at lv_bind / lv_workspace_bytes)
     // slot order of `force`: B (ids in velB) after lv_compute_forces, A after lv_step
     bool force_order_b = true;
     lv_type types[LV_MAX_TYPES];
@@ -115,13 +116,26 @@ int derive_grid(lv_sim *s)
 struct Layout {
     size_t posA, velA, posB, velB, force, key_in, key_out, val_in, val_out, cell_off, sort_temp,
         sort_temp_bytes, st, staging, cell_cnt, scan_tile, scan_ticket, posP, list, list_rows,
-        pos_ref, total;
+        list_off, pos_ref, total;
 };
+
+// Pool of the skin list in rows of 32 entries: list_cap entries per NP on average (any warp may
+// use any share of it); automatic: 1024 entries per NP, at most 2 GiB.
+size_t list_pool_rows_of(const lv_sim *s)
+{
+    if (s->list_cap == 0) return 0;
+    const size_t n = (size_t)(s->n > 0 ? s->n : 1);
+    size_t entries = s->list_cap > 0 ? n * (size_t)s->list_cap : n * 1024;
+    if (s->list_cap < 0 && entries > ((size_t)1 << 29)) entries = (size_t)1 << 29;
+    const size_t rows = (entries + 31) / 32 + 4;
+    return rows > 0xfffffff0ull ? 0xfffffff0ull : rows;
+}
 
 Layout layout_of(const lv_sim *s)
 {
     Layout L;
     const size_t n = (size_t)(s->n > 0 ? s->n : 1);
+    const size_t pool_rows = list_pool_rows_of(s);
     size_t o = 0;
     auto take = [&](size_t bytes) { size_t at = o; o = align_up(o + bytes); return at; };
     L.posA = take(16 * n); L.velA = take(16 * n);
@@ -142,9 +156,10 @@ Layout layout_of(const lv_sim *s)
     L.staging = take(28 * n > 65600 ? 28 * n : 65600);
     L.posP = take(16 * (n + 4));   // pair-interleaved copy of posB + dummy slots (LV_FORCE_PACKED)
     const size_t n_warps = ((n + 127) / 128) * 4;      // warps of the 128-thread force launches
-    L.list = take(s->list_cap > 0 ? 4 * n_warps * 32 * (size_t)s->list_cap : 0);
-    L.list_rows = take(s->list_cap > 0 ? 4 * n_warps : 0);
-    L.pos_ref = take(s->list_cap > 0 ? 16 * n : 0);
+    L.list = take(128 * pool_rows);
+    L.list_rows = take(s->list_cap != 0 ? 4 * n_warps : 0);
+    L.list_off = take(s->list_cap != 0 ? 4 * n_warps : 0);
+    L.pos_ref = take(s->list_cap != 0 ? 16 * n : 0);
     L.total = o;
     return L;
 }
@@ -160,6 +175,7 @@ void derive_tables(lv_sim *s)
     d.n_scan_tiles = (uint32_t)(((size_t)d.n_cells + 1 + kScanTile - 1) / kScanTile);
     d.wall_mode = s->wall_mode;
     d.list_cap = s->list_cap;
+    d.list_pool_rows = (uint32_t)list_pool_rows_of(s);
     d.skin = (float)s->skin;
     {   // rebuild once an NP is farther than half the skin (less 0.1 % for fp32 rounding) from its build position
         const double hs = 0.5 * s->skin * (1.0 - 1e-3);
@@ -221,7 +237,10 @@ int enqueue_stage(lv_sim *s, int stage, bool list_step = false)
             LV_CUDA(s, lvk_rank_gather(s->dev, s->bufs, false, true, s->stream));
             LV_CUDA(s, lvk_list_build(s->dev, s->bufs, s->stream));
             break;
-        case 3: LV_CUDA(s, lvk_pair_force_list(s->dev, s->bufs, s->stream)); break;
+        case 3:
+            LV_CUDA(s, lvk_pair_force_list(s->dev, s->bufs, s->stream));
+            LV_CUDA(s, lvk_pair_force_fallback(s->dev, s->bufs, s->stream));    // only while the list does not fit
+            break;
         default: LV_CUDA(s, lvk_update_list(s->dev, s->bufs, s->stream)); break;
         }
         return LV_OK;
@@ -276,7 +295,7 @@ int enqueue_rebuild_and_forces(lv_sim *s)
 
 int enqueue_step(lv_sim *s)
 {
-    if (s->list_cap > 0) {
+    if (s->list_cap != 0) {
         for (int k = 0; k < LV_N_STAGES; ++k) {
             int rc = enqueue_stage(s, k, true);
             if (rc != LV_OK) return rc;
@@ -293,7 +312,7 @@ int enqueue_step_timed(lv_sim *s, cudaEvent_t *ev)
 {
     LV_CUDA(s, cudaEventRecord(ev[0], s->stream));
     for (int k = 0; k < LV_N_STAGES; ++k) {
-        int rc = enqueue_stage(s, k, s->list_cap > 0);
+        int rc = enqueue_stage(s, k, s->list_cap != 0);
         if (rc != LV_OK) return rc;
         LV_CUDA(s, cudaEventRecord(ev[k + 1], s->stream));
     }
@@ -477,11 +496,31 @@ int lv_set_option(lv_sim *s, int option, int value)
 
 int lv_set_neighbour_list(lv_sim *s, double skin, int capacity)
 {
-    if (!s || !(skin >= 0.0) || capacity < 0 || capacity > (1 << 16)) return LV_E_ARG;
+    if (!s || !std::isfinite(skin) || capacity < -1 || capacity > (1 << 16)) return LV_E_ARG;
     if (s->bound) return LV_E_ORDER;
-    if (capacity > 0 && !(skin > 0.0)) return LV_E_ARG;
-    s->skin = capacity > 0 ? skin : 0.0;
+    if (capacity != 0 && !(skin > 0.0)) {       // automatic skin: a tenth of the smallest cut-off
+        if (!s->types_set) return LV_E_ORDER;
+        double rmin = s->rcut[0];
+        for (int a = 0; a < s->n_types; ++a)
+            for (int b = 0; b < s->n_types; ++b) rmin = std::fmin(rmin, s->rcut[a * LV_MAX_TYPES + b]);
+        skin = 0.1 * rmin;
+    }
+    s->skin = capacity != 0 ? skin : 0.0;
     s->list_cap = capacity;
+    return LV_OK;
+}
+
+int lv_get_list_stats(lv_sim *s, int64_t *out4)
+{
+    if (!s || !out4) return LV_E_ARG;
+    if (!s->bound) return LV_E_ORDER;
+    LvDevState h;
+    LV_CUDA(s, cudaMemcpyAsync(&h, s->bufs.st, sizeof(h), cudaMemcpyDeviceToHost, s->stream));
+    LV_CUDA(s, cudaStreamSynchronize(s->stream));
+    out4[0] = (int64_t)h.n_rebuilds;
+    out4[1] = (int64_t)h.list_rows_used * 32;
+    out4[2] = (int64_t)h.n_fallback;
+    out4[3] = (int64_t)s->dev.list_pool_rows * 32;
     return LV_OK;
 }
 
@@ -509,7 +548,7 @@ int lv_bind(lv_sim *s, void *workspace_dev, size_t workspace_bytes, void *cuda_s
     if (!s) return LV_E_ARG;
     if (!s->types_set || !s->sched_set) return LV_E_ORDER;
     if (s->bound) return LV_E_ORDER;
-    if (s->list_cap > 0 && s->sort_mode != LV_SORT_COUNTING) return LV_E_ARG;
+    if (s->list_cap != 0 && s->sort_mode != LV_SORT_COUNTING) return LV_E_ARG;
     int rc = derive_grid(s);
     if (rc != LV_OK) return rc;
     const Layout L = layout_of(s);
@@ -533,6 +572,7 @@ int lv_bind(lv_sim *s, void *workspace_dev, size_t workspace_bytes, void *cuda_s
     B.posP = (float *)(w + L.posP);
     B.list = (uint32_t *)(w + L.list);
     B.list_rows = (uint32_t *)(w + L.list_rows);
+    B.list_off = (uint32_t *)(w + L.list_off);
     B.pos_ref = (float4 *)(w + L.pos_ref);
     s->ws_bytes = L.total;
     s->stream = (cudaStream_t)cuda_stream;
@@ -875,7 +915,7 @@ int lv_get_state(lv_sim *s, float *pos_xyz, float *vel_xyz, int32_t *type, doubl
     if (R) *R = lv_radius_of(s->sched_mode, s->R0, s->R1, s->sched_steps, h.step);
     if (h.status & LV_ST_BAD_TYPE) return LV_E_ARG;
     if (h.status & LV_ST_NONFINITE) return LV_E_NONFINITE;
-    return (h.status & LV_ST_LIST_OVERFLOW) ? LV_E_CAPACITY : LV_OK;
+    return LV_OK;          // LV_ST_LIST_OVERFLOW is a warning: those steps ran on the cell kernel
 }
 
 int lv_get_forces(lv_sim *s, float *force_xyz, int32_t *neigh_count, int on_device)
@@ -957,7 +997,7 @@ int lv_step_profiled(lv_sim *s, float *ms_out)
     cudaError_t e = cudaSuccess;
     e = cudaEventRecord(ev[0], s->stream);
     for (int k = 0; k < LV_N_STAGES && e == cudaSuccess && rc == LV_OK; ++k) {
-        rc = enqueue_stage(s, k, s->list_cap > 0);
+        rc = enqueue_stage(s, k, s->list_cap != 0);
         if (rc == LV_OK) e = cudaEventRecord(ev[k + 1], s->stream);
     }
     if (e == cudaSuccess) e = cudaStreamSynchronize(s->stream);
@@ -1056,7 +1096,7 @@ const char *lv_strerror(int code)
     case LV_E_ARG: return "bad argument";
     case LV_E_ORDER: return "call order violated";
     case LV_E_WORKSPACE: return "workspace too small or misaligned";
-    case LV_E_CAPACITY: return "skin neighbour list overflowed: raise the capacity";
+    case LV_E_CAPACITY: return "skin neighbour list pool exceeded (reserved; a warning since 0.2: those steps use the cells)";
     case LV_E_CUDA: return "CUDA runtime error";
     case LV_E_NONFINITE: return "non-finite position or velocity";
     case LV_E_NOMEM: return "host allocation failed";

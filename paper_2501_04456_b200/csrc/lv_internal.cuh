@@ -49,7 +49,8 @@ struct LvDev {
     uint32_t seed_lo, seed_hi;
     uint32_t n_scan_tiles;   // tiles of the cell-count scan (counting sort)
     // skin neighbour list (lv_set_neighbour_list); list_cap = 0: off
-    int32_t list_cap;        // entries per NP
+    int32_t list_cap;        // != 0: list on
+    uint32_t list_pool_rows; // pool of the list in rows (32 entries = 128 bytes each)
     float skin;              // list radius = r_c,ab + skin
     float half_skin2;        // rebuild when an NP has moved farther than this (squared) since the build
     // LV_FORCE_TILE: a target of type a more than this many cells of its grid along x from a
@@ -67,7 +68,13 @@ struct LvDevState {
     // rebuild[n & 1], clears it for step n + 2.
     unsigned int rebuild[2];
     unsigned int n_rebuilds;   // rebuilds since lv_set_state
-    unsigned int pad;
+    // skin list: 1 = the list of the last rebuild fits the pool and is in use; 0 = the pool was
+    // too small at the last count -- steps rebuild the cells and use the cell kernel until a
+    // later count (every 64th step) fits again
+    unsigned int list_ok;
+    unsigned int list_rows_used;   // rows of the pool the last build needed
+    unsigned int n_fallback;       // steps taken on the cell kernel since lv_set_state
+    unsigned int pad[3];
 };
 
 struct LvBufs {
@@ -90,11 +97,13 @@ struct LvBufs {
     // 32 bytes {x0, x1, y0, y1, z0, z1, w0, w1}; slots n .. 2*ceil(n/2)+1 are dummies far
     // outside every cut-off.  Written by the gather only when that kernel is selected.
     float *posP;
-    // skin neighbour list: warp w of 32 consecutive slots owns list[(w * cap + t) * 32 + lane],
-    // t < list_rows[w] (entries past an NP's own count hold its own slot); pos_ref = positions
-    // at the last build.
+    // skin neighbour list: warp w of 32 consecutive slots owns the tile
+    // list[(list_off[w] + t) * 32 + lane], t < list_rows[w] = the longest list of its lanes
+    // (entries past an NP's own count hold its own slot); list_off = exclusive scan of
+    // list_rows; pos_ref = positions at the last build.
     uint32_t *list;
     uint32_t *list_rows;
+    uint32_t *list_off;
     float4 *pos_ref;
 };
 
@@ -124,7 +133,10 @@ cudaError_t lvk_scan_cells(const LvDev &P, const LvBufs &B, bool guarded, cudaSt
 cudaError_t lvk_place(const LvDev &P, const LvBufs &B, bool guarded, cudaStream_t st);
 cudaError_t lvk_rank_gather(const LvDev &P, const LvBufs &B, bool packed, bool guarded, cudaStream_t st);
 // skin list: build from the cell structures (guarded), force from the list, update in list order
+// count (rows per warp) -> scan (tile offsets, pool check) -> fill, all guarded
 cudaError_t lvk_list_build(const LvDev &P, const LvBufs &B, cudaStream_t st);
+// cell kernel of a list step: runs only while the list does not fit its pool
+cudaError_t lvk_pair_force_fallback(const LvDev &P, const LvBufs &B, cudaStream_t st);
 cudaError_t lvk_pair_force_list(const LvDev &P, const LvBufs &B, cudaStream_t st);
 cudaError_t lvk_update_list(const LvDev &P, const LvBufs &B, cudaStream_t st);
 cudaError_t lvk_keys_sorted(const LvDev &P, const LvBufs &B, uint32_t *out, cudaStream_t st);

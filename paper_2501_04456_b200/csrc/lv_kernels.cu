@@ -522,11 +522,17 @@ __global__ void __launch_bounds__(kSThreads, LV_S_MINBLOCKS)
 k_pair_force_s(const __grid_constant__ LvDev P, const float4 *__restrict__ pos,
                const uint32_t *__restrict__ off, float4 *__restrict__ force,
                const float *__restrict__ posP, uint32_t *__restrict__ list,
-               uint32_t *__restrict__ list_rows, LvDevState *st)
+               uint32_t *__restrict__ list_rows, const uint32_t *__restrict__ list_off, LvDevState *st)
 {
     constexpr bool kPacked = kMode == 1;
-    constexpr bool kList = kMode == 2;
+    constexpr bool kList = kMode >= 2;          // 2: fill the list, 3: count its rows
+    constexpr bool kCount = kMode == 3;
     if (kList && skipped(st)) return;
+    // a list that did not fit its pool is counted again only every 64th step
+    if (kCount && st->list_ok == 0u && (st->step & 63) != 0) return;
+    if (kMode == 2 && st->list_ok == 0u) return;
+    // cell kernel of a list step (st given): only while the list is not in use
+    if (kMode == 0 && st != nullptr && st->list_ok != 0u) return;
     __shared__ LvPair s_pair[LV_MAX_TYPES * LV_MAX_TYPES];
     __shared__ int8_t s_w[LV_MAX_TYPES * LV_MAX_TYPES];
     __shared__ uint2 s_seg[kSegCap * kSThreads];
@@ -540,8 +546,8 @@ k_pair_force_s(const __grid_constant__ LvDev P, const float4 *__restrict__ pos,
     const bool live = i >= 0;
     const uint32_t self = live ? (uint32_t)i : 0u;
     // list mode: the lane's column of its warp's tile, and whether it overflowed
-    uint32_t *col = kList ? list + ((size_t)(gtid >> 5) * P.list_cap) * 32u + (gtid & 31) : nullptr;
-    bool overflow = false;
+    // fill mode: the lane's column of its warp's tile (list_off = exclusive scan of the rows)
+    uint32_t *col = kMode == 2 ? list + (size_t)list_off[gtid >> 5] * 32u + (gtid & 31) : nullptr;
     const float4 pi = pos[self];
     const int a = live ? __float_as_int(pi.w) : 0;
     const LvPair *pair_a = s_pair + a * LV_MAX_TYPES;
@@ -585,9 +591,8 @@ k_pair_force_s(const __grid_constant__ LvDev P, const float4 *__restrict__ pos,
                 const bool in = r2 < rc2 && jj[u] != self;           // fp32 contract #2
                 if (kList) {
                     if (in) {
-                        if (cnt < P.list_cap) col[(size_t)cnt * 32u] = jj[u];
-                        else overflow = true;
-                        cnt += cnt < P.list_cap ? 1 : 0;
+                        if (!kCount) col[(size_t)cnt * 32u] = jj[u];
+                        ++cnt;
                     }
                     continue;
                 }
@@ -806,10 +811,12 @@ k_pair_force_s(const __grid_constant__ LvDev P, const float4 *__restrict__ pos,
         // rows of the tile = the longest column; shorter columns are filled with the lane's
         // own slot, which the force kernel rejects by j != i
         const int rows = __reduce_max_sync(kFull, cnt);
-        for (int t = cnt; t < rows; ++t) col[(size_t)t * 32u] = self;
-        if ((gtid & 31) == 0) list_rows[gtid >> 5] = (uint32_t)rows;
-        if (overflow) atomicOr(&st->status, LV_ST_LIST_OVERFLOW);
-        if (gtid == 0) st->n_rebuilds += 1u;
+        if (kCount) {
+            if ((gtid & 31) == 0) list_rows[gtid >> 5] = (uint32_t)rows;
+        } else {
+            for (int t = cnt; t < rows; ++t) col[(size_t)t * 32u] = self;
+            if (gtid == 0) st->n_rebuilds += 1u;
+        }
         return;
     }
     if (live) force[i] = make_float4(fx, fy, fz, __int_as_float(cnt));
@@ -827,9 +834,10 @@ template <bool kCharged>
 __global__ void __launch_bounds__(kSThreads)
 k_pair_force_list(const __grid_constant__ LvDev P, const float4 *__restrict__ posA,
                   const float4 *__restrict__ posB, const uint32_t *__restrict__ list,
-                  const uint32_t *__restrict__ list_rows, float4 *__restrict__ force,
-                  const LvDevState *st)
+                  const uint32_t *__restrict__ list_rows, const uint32_t *__restrict__ list_off,
+                  float4 *__restrict__ force, const LvDevState *st)
 {
+    if (st->list_ok == 0u) return;          // the cell kernel takes this step
     __shared__ LvPair s_pair[LV_MAX_TYPES * LV_MAX_TYPES];
     for (int t = threadIdx.x; t < LV_MAX_TYPES * LV_MAX_TYPES; t += kSThreads) s_pair[t] = P.pair[t];
     __syncthreads();
@@ -840,7 +848,7 @@ k_pair_force_list(const __grid_constant__ LvDev P, const float4 *__restrict__ po
     const uint32_t self = live ? (uint32_t)i : 0u;
     const float4 pi = pos[self];
     const LvPair *pair_a = s_pair + (live ? __float_as_int(pi.w) : 0) * LV_MAX_TYPES;
-    const uint32_t *col = list + ((size_t)(gtid >> 5) * P.list_cap) * 32u + (gtid & 31);
+    const uint32_t *col = list + (size_t)list_off[gtid >> 5] * 32u + (gtid & 31);
     const int rows = (int)list_rows[gtid >> 5];
     float fx = 0.f, fy = 0.f, fz = 0.f;
     int cnt = 0;
@@ -948,7 +956,13 @@ k_update(const __grid_constant__ LvDev P, const float4 *__restrict__ posB_,
         if (atomicAdd(&st->ticket, 1u) == gridDim.x - 1) {
             st->ticket = 0u;
             st->step = n0 + 1;
-            if (kList) st->rebuild[n0 & 1] = 0u;       // ... and this step's rebuild flag
+            if (kList) {
+                st->rebuild[n0 & 1] = 0u;              // ... and this step's rebuild flag
+                if (st->list_ok == 0u) {               // on the cell kernel: every step rebuilds the cells
+                    st->rebuild[(n0 + 1) & 1] = 1u;
+                    st->n_fallback += 1u;
+                }
+            }
         }
     }
     __syncthreads();
@@ -1042,6 +1056,9 @@ k_pack_state(int n, int n_types, const float *__restrict__ pos, const float *__r
         st->rebuild[step & 1] = 1u;            // skin list: the first step builds it
         st->rebuild[(step + 1) & 1] = 0u;
         st->n_rebuilds = 0u;
+        st->list_ok = 1u;
+        st->list_rows_used = 0u;
+        st->n_fallback = 0u;
     }
     if (i >= n) return;
     int a = type[i];
@@ -1536,28 +1553,69 @@ cudaError_t lvk_pair_force(const LvDev &P, const LvBufs &B, int variant, cudaStr
         if (variant == 3) {
             if (charged)
                 k_pair_force_s<true, 1><<<blocks, kSThreads, 0, st>>>(P, B.posB, B.cell_off, B.force,
-                                                                      B.posP, nullptr, nullptr, nullptr);
+                                                                      B.posP, nullptr, nullptr, nullptr, nullptr);
             else
                 k_pair_force_s<false, 1><<<blocks, kSThreads, 0, st>>>(P, B.posB, B.cell_off, B.force,
-                                                                       B.posP, nullptr, nullptr, nullptr);
+                                                                       B.posP, nullptr, nullptr, nullptr, nullptr);
         } else {
             if (charged)
                 k_pair_force_s<true, 0><<<blocks, kSThreads, 0, st>>>(P, B.posB, B.cell_off, B.force,
-                                                                      nullptr, nullptr, nullptr, nullptr);
+                                                                      nullptr, nullptr, nullptr, nullptr, nullptr);
             else
                 k_pair_force_s<false, 0><<<blocks, kSThreads, 0, st>>>(P, B.posB, B.cell_off, B.force,
-                                                                       nullptr, nullptr, nullptr, nullptr);
+                                                                       nullptr, nullptr, nullptr, nullptr, nullptr);
         }
     }
     return cudaGetLastError();
 }
 
-// skin list: tiles are indexed by the launch's warp id, so build and force use the same grid
+// Exclusive scan of the rows per warp -> tile offsets; decides whether the list fits its pool
+// (one block: the table has n / 32 entries).
+namespace {
+constexpr int kLScanThreads = 1024;
+__global__ void __launch_bounds__(kLScanThreads)
+k_list_scan(int n_warps, uint32_t pool_rows, const uint32_t *__restrict__ rows, uint32_t *__restrict__ offs,
+            LvDevState *st)
+{
+    if (skipped(st)) return;
+    if (st->list_ok == 0u && (st->step & 63) != 0) return;       // not counted this step
+    __shared__ unsigned long long s_sum[kLScanThreads];
+    const int per = (n_warps + kLScanThreads - 1) / kLScanThreads;
+    const int lo = threadIdx.x * per, hi = min(lo + per, n_warps);
+    unsigned long long sum = 0ull;
+    for (int k = lo; k < hi; ++k) sum += rows[k];
+    s_sum[threadIdx.x] = sum;
+    __syncthreads();
+    for (int d = 1; d < kLScanThreads; d <<= 1) {                 // inclusive scan of the chunk sums
+        const unsigned long long v = threadIdx.x >= d ? s_sum[threadIdx.x - d] : 0ull;
+        __syncthreads();
+        s_sum[threadIdx.x] += v;
+        __syncthreads();
+    }
+    const unsigned long long total = s_sum[kLScanThreads - 1];
+    const bool fits = total <= (unsigned long long)pool_rows;
+    if (fits) {
+        unsigned long long run = s_sum[threadIdx.x] - sum;
+        for (int k = lo; k < hi; ++k) { offs[k] = (uint32_t)run; run += rows[k]; }
+    }
+    if (threadIdx.x == 0) {
+        st->list_ok = fits ? 1u : 0u;
+        st->list_rows_used = total > 0xffffffffull ? 0xffffffffu : (uint32_t)total;
+        if (!fits) atomicOr(&st->status, LV_ST_LIST_OVERFLOW);
+    }
+}
+}  // namespace
+
+// skin list: tiles are indexed by the launch's warp id, so count, fill and force use the same grid
 cudaError_t lvk_list_build(const LvDev &P, const LvBufs &B, cudaStream_t st)
 {
     const int blocks = (P.n + kSThreads - 1) / kSThreads;
-    k_pair_force_s<false, 2><<<blocks, kSThreads, 0, st>>>(P, B.posB, B.cell_off, nullptr, nullptr,
-                                                           B.list, B.list_rows, B.st);
+    k_pair_force_s<false, 3><<<blocks, kSThreads, 0, st>>>(P, B.posB, B.cell_off, nullptr, nullptr, nullptr,
+                                                           B.list_rows, nullptr, B.st);
+    k_list_scan<<<1, kLScanThreads, 0, st>>>(blocks * (kSThreads / 32), P.list_pool_rows, B.list_rows,
+                                             B.list_off, B.st);
+    k_pair_force_s<false, 2><<<blocks, kSThreads, 0, st>>>(P, B.posB, B.cell_off, nullptr, nullptr, B.list,
+                                                           B.list_rows, B.list_off, B.st);
     return cudaGetLastError();
 }
 
@@ -1566,10 +1624,22 @@ cudaError_t lvk_pair_force_list(const LvDev &P, const LvBufs &B, cudaStream_t st
     const int blocks = (P.n + kSThreads - 1) / kSThreads;
     if (lvk_any_charge(P))
         k_pair_force_list<true><<<blocks, kSThreads, 0, st>>>(P, B.posA, B.posB, B.list, B.list_rows,
-                                                              B.force, B.st);
+                                                              B.list_off, B.force, B.st);
     else
         k_pair_force_list<false><<<blocks, kSThreads, 0, st>>>(P, B.posA, B.posB, B.list, B.list_rows,
-                                                               B.force, B.st);
+                                                               B.list_off, B.force, B.st);
+    return cudaGetLastError();
+}
+
+cudaError_t lvk_pair_force_fallback(const LvDev &P, const LvBufs &B, cudaStream_t st)
+{
+    const int blocks = (P.n + kSThreads - 1) / kSThreads;
+    if (lvk_any_charge(P))
+        k_pair_force_s<true, 0><<<blocks, kSThreads, 0, st>>>(P, B.posB, B.cell_off, B.force, nullptr, nullptr,
+                                                              nullptr, nullptr, B.st);
+    else
+        k_pair_force_s<false, 0><<<blocks, kSThreads, 0, st>>>(P, B.posB, B.cell_off, B.force, nullptr, nullptr,
+                                                               nullptr, nullptr, B.st);
     return cudaGetLastError();
 }
 

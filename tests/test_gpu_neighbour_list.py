@@ -126,14 +126,75 @@ def test_split_invariance_and_restart(B):
     a.close(); b.close()
 
 
-def test_overflow_is_reported(B):
+def test_pool_too_small_falls_back_to_the_cells(B):
+    """A pool the list cannot fit (8 entries per NP for ~50 neighbours): no error, the warning
+    bit is raised and every step runs on the cell kernel -- the same kernels as the default
+    path, so counts, forces and the trajectory are BIT-identical to a run without the list."""
     w = W.make_workload("C4", 19999)              # ~50 neighbours per NP
-    sim = B.Simulation.from_workload(w, cells_per_cut=[2], neighbour_list=(0.2, 8))
+    lst = B.Simulation.from_workload(w, cells_per_cut=[2], neighbour_list=(0.2, 8))
+    cel = B.Simulation.from_workload(w, cells_per_cut=[2])
+    lst.step(1); cel.step(1)
+    Fl, cl = lst.get_forces()
+    Fc, cc = cel.get_forces()
+    assert np.array_equal(cl, cc) and np.array_equal(Fl, Fc) and cc.sum() > 0
+    assert lst.status() == B.ST_LIST_OVERFLOW
+    lst.step(70); cel.step(70)                    # past a re-count (every 64th step)
+    a, b = lst.get_state(), cel.get_state()       # no LV_E_CAPACITY any more
+    assert np.array_equal(a[0], b[0]) and np.array_equal(a[1], b[1]) and a[4] == b[4] == 71
+    st = lst.list_stats()
+    assert st["fallback_steps"] == 71 and st["entries_used"] > st["pool_entries"]
+    lst.close(); cel.close()
+
+
+def test_list_follows_a_shrinking_droplet_into_the_fallback(B, orc):
+    """The pool fits the dilute start of C2 and not its crowded end: the run starts on the list,
+    changes over to the cells on the device when a rebuild no longer fits, keeps the oracle
+    tolerance over the first 100 steps, stays split-invariant across the change-over, and its
+    counts at the end equal a fresh cell rebuild of the same state."""
+    w = W.make_workload("C2", 8191)
+    p = orc.params_from_workload(w)
+    mk = lambda: B.Simulation.from_workload(w, cells_per_cut=[2, 2], neighbour_list=(0.4, 96))
+    a, b = mk(), mk()
+    a.step(100)
+    x, v, t, R, st = a.get_state()
+    xo, vo, bad = orc.step(p, w.pos, w.vel, w.type, step0=0, nsteps=100)
+    assert bad == 0 and np.linalg.norm(x.astype(np.float64) - xo, axis=1).max() <= 1e-3 * R
+    assert a.list_stats()["fallback_steps"] == 0
+    a.step(6900)
+    b.step(3300); b.step(1); b.step(3699)
+    xa, va, ta, Ra, sa = a.get_state()
+    xb, vb, _, _, sb = b.get_state()
+    assert sa == sb == 7000 and np.array_equal(xa, xb) and np.array_equal(va, vb)
+    st = a.list_stats()
+    assert 0 < st["fallback_steps"] < 7000 and st["rebuilds"] > 1
+    assert a.status() & B.ST_LIST_OVERFLOW
+    cel = B.Simulation.from_workload(w, cells_per_cut=[2, 2], load_state=False)
+    cel.set_state(xa, va, ta, sa)
+    cel.compute_forces()
+    Fc, cc = cel.get_forces()
+    a.step(1)
+    Fl, cl = a.get_forces()
+    assert np.array_equal(cl, cc) and cc.mean() > 60
+    a.close(); b.close(); cel.close()
+
+
+def test_automatic_skin_and_pool(B, orc):
+    """lv_set_neighbour_list(skin <= 0, capacity = -1): skin = a tenth of the smallest cut-off,
+    pool = 1024 entries per NP; first-step counts bit-exact, 100 steps within tolerance."""
+    w = W.make_workload("C3", 20000)
+    p = orc.params_from_workload(w)
+    Fo, So, co, _ = orc.pair_forces(p, w.pos, w.type, "cells")
+    sim = B.Simulation.from_workload(w, cells_per_cut=[1, 2, 2], neighbour_list=(0.0, -1))
     sim.step(1)
-    assert sim.status() & B.ST_LIST_OVERFLOW
-    with pytest.raises(B.LvError) as e:
-        sim.get_state()
-    assert e.value.code == B.E_CAPACITY
+    Fg, cg = sim.get_forces()
+    assert np.array_equal(cg, co) and force_error(Fg, Fo, So) <= FORCE_TOL
+    sim.step(99)
+    x, v, t, R, st = sim.get_state()
+    xo, vo, bad = orc.step(p, w.pos, w.vel, w.type, step0=0, nsteps=100)
+    assert bad == 0 and np.linalg.norm(x.astype(np.float64) - xo, axis=1).max() <= 1e-3 * R
+    s = sim.list_stats()
+    assert s["pool_entries"] >= 1024 * w.n and s["fallback_steps"] == 0 and 1 <= s["rebuilds"] < 100
+    assert sim.status() == 0
     sim.close()
 
 
