@@ -157,6 +157,9 @@ int lv_set_grid(lv_sim *s, const int32_t *cells_per_cut);
  *                        memory by 1-D bulk copies (TMA), and S lanes per target walk the
  *                        same staged stream (steps i-ii).
  *   LV_OPT_TILE_SUBSTREAMS  S of LV_FORCE_TILE: 1, 2, 4 (default), 8, 16 or 32 lanes per target.
+ *   LV_OPT_LIST_LANES    lanes that share one NP's neighbour list in the list force kernel:
+ *                        1, 2, 4, 8, 16, 32, or 0 (default) = chosen on the device at every
+ *                        rebuild from the mean list length.
  *   LV_OPT_TILE_SPAN     cells along x (of the targets' own grid) a tile may extend beyond
  *                        the cell of its first target; -1 (default): cells_per_cut - 1.
  * Every setting gives bit-identical permutations, offsets and neighbour counts;
@@ -172,6 +175,7 @@ int lv_set_grid(lv_sim *s, const int32_t *cells_per_cut);
 #define LV_FORCE_TILE        4
 #define LV_OPT_TILE_SUBSTREAMS 3
 #define LV_OPT_TILE_SPAN       4
+#define LV_OPT_LIST_LANES      5
 int lv_set_option(lv_sim *s, int option, int value);
 
 /* Persistent "skin" neighbour list.  The paper rebuilds the cells
@@ -187,8 +191,9 @@ int lv_set_option(lv_sim *s, int option, int value);
  *             NP of workspace; a crowded NP may use more than its share); -1: automatic, 1024
  *             entries per NP but at most 2 GiB; 0 (default): the variant is off and every step
  *             rebuilds the cells, as the paper does.
- * The list is built in two passes (count, then fill) into per-warp tiles whose height is the
- * longest list of the warp.  If a rebuild would need more than the pool, nothing is lost: the
+ * The list is built in two passes (count the lengths, scan them, fill): every NP owns one
+ * contiguous run of the pool, and 8, 16 or 32 lanes share an NP in the force kernel (chosen on
+ * the device from the mean length).  If a rebuild would need more than the pool, nothing is lost: the
  * warning bit LV_ST_LIST_OVERFLOW is raised and the steps run on the cell kernel (rebuilding the
  * cells every step) until a later count -- taken every 64th step -- fits again.  The choice
  * depends only on the state and the step index, so lv_step(a); lv_step(b) == lv_step(a + b)
@@ -199,8 +204,8 @@ int lv_set_neighbour_list(lv_sim *s, double skin, int capacity);
  * with the neighbour list on.  Synchronises. */
 int lv_get_rebuild_count(lv_sim *s, int64_t *rebuilds);
 
-/* out4 (host int64[4], written): rebuilds since lv_set_state, list entries (padded tiles) the
- * last count needed, steps taken on the cell kernel because the list did not fit, pool size
+/* out4 (host int64[4], written): rebuilds since lv_set_state, list entries (lengths padded to
+ * a multiple of 4) the last count needed, steps taken on the cell kernel because the list did not fit, pool size
  * in entries.  Synchronises. */
 int lv_get_list_stats(lv_sim *s, int64_t *out4);
 

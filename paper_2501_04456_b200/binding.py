@@ -23,7 +23,7 @@ ST_NONFINITE, ST_OUTSIDE_GRID, ST_LIST_OVERFLOW = 1, 2, 4
 DBG_KEYS, DBG_KEYS_SORTED, DBG_PERM, DBG_CELL_OFFSETS, DBG_IDS_SORTED, DBG_GRID = 1, 2, 3, 4, 5, 6
 E_NONFINITE = -5
 E_CAPACITY = -7
-OPT_SORT, OPT_FORCE_KERNEL, OPT_TILE_SUBSTREAMS, OPT_TILE_SPAN = 1, 2, 3, 4
+OPT_SORT, OPT_FORCE_KERNEL, OPT_TILE_SUBSTREAMS, OPT_TILE_SPAN, OPT_LIST_LANES = 1, 2, 3, 4, 5
 SORT_COUNTING, SORT_RADIX = 0, 1
 FORCE_SIMPLE, FORCE_QUEUED, FORCE_SEGMENTS, FORCE_PACKED, FORCE_TILE = 0, 1, 2, 3, 4
 

@@ -21,7 +21,6 @@ struct lv_sim {
     // skin neighbour list (lv_set_neighbour_list); list_cap = 0: off
     double skin = 0.0;
     int list_cap = 0;               // 0: off; > 0: pool of list_cap entries per NP; -1: automatic pool
-    size_t list_pool_rows = 0;      // pool in rows of 32 entries (derived at lv_bind / lv_workspace_bytes)
     // slot order of `force`: B (ids in velB) after lv_compute_forces, A after lv_step
     bool force_order_b = true;
     lv_type types[LV_MAX_TYPES];
@@ -39,6 +38,7 @@ struct lv_sim {
     int sort_mode = LV_SORT_COUNTING;
     int force_kernel = LV_FORCE_SEGMENTS;
     int tile_substreams = 4;        // LV_OPT_TILE_SUBSTREAMS: lanes per target of LV_FORCE_TILE
+    int list_lanes = 0;             // LV_OPT_LIST_LANES: lanes per NP of the list force kernel (0: automatic)
     int tile_span = -1;             // LV_OPT_TILE_SPAN: cells along x a tile may span beyond its first (-1: k_a - 1)
     lv_grid_info grid;
     int sort_end_bit = 1;
@@ -115,27 +115,26 @@ int derive_grid(lv_sim *s)
 
 struct Layout {
     size_t posA, velA, posB, velB, force, key_in, key_out, val_in, val_out, cell_off, sort_temp,
-        sort_temp_bytes, st, staging, cell_cnt, scan_tile, scan_ticket, posP, list, list_rows,
-        list_off, pos_ref, total;
+        sort_temp_bytes, st, staging, cell_cnt, scan_tile, scan_ticket, posP, list, list_cnt,
+        list_start, list_scan_tile, list_scan_ticket, pos_ref, total;
 };
 
-// Pool of the skin list in rows of 32 entries: list_cap entries per NP on average (any warp may
-// use any share of it); automatic: 1024 entries per NP, at most 2 GiB.
-size_t list_pool_rows_of(const lv_sim *s)
+// Pool of the skin list in entries: list_cap per NP on average (a crowded NP may use more than
+// its share); automatic: 1024 entries per NP, at most 2 GiB.
+size_t list_pool_of(const lv_sim *s)
 {
     if (s->list_cap == 0) return 0;
     const size_t n = (size_t)(s->n > 0 ? s->n : 1);
     size_t entries = s->list_cap > 0 ? n * (size_t)s->list_cap : n * 1024;
     if (s->list_cap < 0 && entries > ((size_t)1 << 29)) entries = (size_t)1 << 29;
-    const size_t rows = (entries + 31) / 32 + 4;
-    return rows > 0xfffffff0ull ? 0xfffffff0ull : rows;
+    entries += 64;
+    return entries > 0xfffffff0ull ? 0xfffffff0ull : entries;
 }
 
 Layout layout_of(const lv_sim *s)
 {
     Layout L;
     const size_t n = (size_t)(s->n > 0 ? s->n : 1);
-    const size_t pool_rows = list_pool_rows_of(s);
     size_t o = 0;
     auto take = [&](size_t bytes) { size_t at = o; o = align_up(o + bytes); return at; };
     L.posA = take(16 * n); L.velA = take(16 * n);
@@ -155,10 +154,11 @@ Layout layout_of(const lv_sim *s)
     // smaller than their largest histogram (8 * 8192 + 64 B)
     L.staging = take(28 * n > 65600 ? 28 * n : 65600);
     L.posP = take(16 * (n + 4));   // pair-interleaved copy of posB + dummy slots (LV_FORCE_PACKED)
-    const size_t n_warps = ((n + 127) / 128) * 4;      // warps of the 128-thread force launches
-    L.list = take(128 * pool_rows);
-    L.list_rows = take(s->list_cap != 0 ? 4 * n_warps : 0);
-    L.list_off = take(s->list_cap != 0 ? 4 * n_warps : 0);
+    L.list = take(4 * list_pool_of(s));
+    L.list_cnt = take(s->list_cap != 0 ? 4 * (n + 1) : 0);
+    L.list_start = take(s->list_cap != 0 ? 4 * (n + 1) : 0);
+    L.list_scan_tile = take(s->list_cap != 0 ? 8 * ((n + 1 + kScanTile - 1) / kScanTile) : 0);
+    L.list_scan_ticket = take(4);
     L.pos_ref = take(s->list_cap != 0 ? 16 * n : 0);
     L.total = o;
     return L;
@@ -175,7 +175,9 @@ void derive_tables(lv_sim *s)
     d.n_scan_tiles = (uint32_t)(((size_t)d.n_cells + 1 + kScanTile - 1) / kScanTile);
     d.wall_mode = s->wall_mode;
     d.list_cap = s->list_cap;
-    d.list_pool_rows = (uint32_t)list_pool_rows_of(s);
+    d.list_pool = (uint32_t)list_pool_of(s);
+    d.list_lanes_forced = s->list_lanes;
+    d.n_list_tiles = (uint32_t)(((size_t)(s->n > 0 ? s->n : 1) + 1 + kScanTile - 1) / kScanTile);
     d.skin = (float)s->skin;
     {   // rebuild once an NP is farther than half the skin (less 0.1 % for fp32 rounding) from its build position
         const double hs = 0.5 * s->skin * (1.0 - 1e-3);
@@ -485,6 +487,10 @@ int lv_set_option(lv_sim *s, int option, int value)
         if (value < 1 || value > 32 || (value & (value - 1)) != 0) return LV_E_ARG;
         s->tile_substreams = value;
         return LV_OK;
+    case LV_OPT_LIST_LANES:
+        if (value < 0 || value > 32 || (value & (value - 1)) != 0) return LV_E_ARG;
+        s->list_lanes = value;
+        return LV_OK;
     case LV_OPT_TILE_SPAN:
         if (value < -1 || value > 1024) return LV_E_ARG;
         s->tile_span = value;
@@ -518,9 +524,9 @@ int lv_get_list_stats(lv_sim *s, int64_t *out4)
     LV_CUDA(s, cudaMemcpyAsync(&h, s->bufs.st, sizeof(h), cudaMemcpyDeviceToHost, s->stream));
     LV_CUDA(s, cudaStreamSynchronize(s->stream));
     out4[0] = (int64_t)h.n_rebuilds;
-    out4[1] = (int64_t)h.list_rows_used * 32;
+    out4[1] = (int64_t)h.list_used;
     out4[2] = (int64_t)h.n_fallback;
-    out4[3] = (int64_t)s->dev.list_pool_rows * 32;
+    out4[3] = (int64_t)s->dev.list_pool;
     return LV_OK;
 }
 
@@ -571,8 +577,10 @@ int lv_bind(lv_sim *s, void *workspace_dev, size_t workspace_bytes, void *cuda_s
     B.scan_ticket = (unsigned int *)(w + L.scan_ticket);
     B.posP = (float *)(w + L.posP);
     B.list = (uint32_t *)(w + L.list);
-    B.list_rows = (uint32_t *)(w + L.list_rows);
-    B.list_off = (uint32_t *)(w + L.list_off);
+    B.list_cnt = (uint32_t *)(w + L.list_cnt);
+    B.list_start = (uint32_t *)(w + L.list_start);
+    B.list_scan_tile = (unsigned long long *)(w + L.list_scan_tile);
+    B.list_scan_ticket = (unsigned int *)(w + L.list_scan_ticket);
     B.pos_ref = (float4 *)(w + L.pos_ref);
     s->ws_bytes = L.total;
     s->stream = (cudaStream_t)cuda_stream;

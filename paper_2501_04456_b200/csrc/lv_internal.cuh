@@ -50,7 +50,9 @@ struct LvDev {
     uint32_t n_scan_tiles;   // tiles of the cell-count scan (counting sort)
     // skin neighbour list (lv_set_neighbour_list); list_cap = 0: off
     int32_t list_cap;        // != 0: list on
-    uint32_t list_pool_rows; // pool of the list in rows (32 entries = 128 bytes each)
+    uint32_t list_pool;      // pool of the list in entries (4 bytes each)
+    uint32_t n_list_tiles;   // tiles of the scan over the list lengths
+    int32_t list_lanes_forced;   // LV_OPT_LIST_LANES: 0 = chosen on the device
     float skin;              // list radius = r_c,ab + skin
     float half_skin2;        // rebuild when an NP has moved farther than this (squared) since the build
     // LV_FORCE_TILE: a target of type a more than this many cells of its grid along x from a
@@ -72,9 +74,11 @@ struct LvDevState {
     // too small at the last count -- steps rebuild the cells and use the cell kernel until a
     // later count (every 64th step) fits again
     unsigned int list_ok;
-    unsigned int list_rows_used;   // rows of the pool the last build needed
+    unsigned int list_lanes;       // lanes that share one NP's list in the force kernel (8, 16 or 32)
     unsigned int n_fallback;       // steps taken on the cell kernel since lv_set_state
-    unsigned int pad[3];
+    unsigned int pad;
+    unsigned long long list_total; // entries counted by the count pass that is under way
+    unsigned long long list_used;  // entries the last count needed
 };
 
 struct LvBufs {
@@ -97,13 +101,15 @@ struct LvBufs {
     // 32 bytes {x0, x1, y0, y1, z0, z1, w0, w1}; slots n .. 2*ceil(n/2)+1 are dummies far
     // outside every cut-off.  Written by the gather only when that kernel is selected.
     float *posP;
-    // skin neighbour list: warp w of 32 consecutive slots owns the tile
-    // list[(list_off[w] + t) * 32 + lane], t < list_rows[w] = the longest list of its lanes
-    // (entries past an NP's own count hold its own slot); list_off = exclusive scan of
-    // list_rows; pos_ref = positions at the last build.
+    // skin neighbour list: the NP at sorted slot i owns list[list_start[i] .. list_start[i + 1]),
+    // its neighbours' slots in walk order, padded to a multiple of 4 entries with its own slot;
+    // list_cnt = padded lengths (input of the scan, zero between builds), list_start = their
+    // exclusive scan; pos_ref = positions at the last build.
     uint32_t *list;
-    uint32_t *list_rows;
-    uint32_t *list_off;
+    uint32_t *list_cnt;      // [n + 1]
+    uint32_t *list_start;    // [n + 1]
+    unsigned long long *list_scan_tile;
+    unsigned int *list_scan_ticket;
     float4 *pos_ref;
 };
 

@@ -147,9 +147,11 @@ constexpr int kScanThreads = kScanTile / kScanItems;
 __global__ void __launch_bounds__(kScanThreads)
 k_scan_cells(uint32_t n_items, uint32_t *__restrict__ cnt, uint32_t *__restrict__ off,
              volatile unsigned long long *scan_tile, unsigned int *scan_ticket,
-             const LvDevState *guard)
+             const LvDevState *guard, const LvDevState *list_guard)
 {
     if (skipped(guard)) return;
+    // scan of the list lengths: a list that did not fit is counted again only every 64th step
+    if (list_guard != nullptr && list_guard->list_ok == 0u && (list_guard->step & 63) != 0) return;
     __shared__ uint32_t s_warp[kScanThreads / 32];
     __shared__ uint32_t s_tile, s_excl;
     if (threadIdx.x == 0) s_tile = atomicAdd(scan_ticket, 1u);   // tiles start in ticket order
@@ -522,7 +524,9 @@ __global__ void __launch_bounds__(kSThreads, LV_S_MINBLOCKS)
 k_pair_force_s(const __grid_constant__ LvDev P, const float4 *__restrict__ pos,
                const uint32_t *__restrict__ off, float4 *__restrict__ force,
                const float *__restrict__ posP, uint32_t *__restrict__ list,
-               uint32_t *__restrict__ list_rows, const uint32_t *__restrict__ list_off, LvDevState *st)
+               uint32_t *__restrict__ list_cnt, const uint32_t *__restrict__ list_start,
+               unsigned long long *__restrict__ list_scan_tile, unsigned int *__restrict__ list_scan_ticket,
+               LvDevState *st)
 {
     constexpr bool kPacked = kMode == 1;
     constexpr bool kList = kMode >= 2;          // 2: fill the list, 3: count its rows
@@ -546,8 +550,14 @@ k_pair_force_s(const __grid_constant__ LvDev P, const float4 *__restrict__ pos,
     const bool live = i >= 0;
     const uint32_t self = live ? (uint32_t)i : 0u;
     // list mode: the lane's column of its warp's tile, and whether it overflowed
-    // fill mode: the lane's column of its warp's tile (list_off = exclusive scan of the rows)
-    uint32_t *col = kMode == 2 ? list + (size_t)list_off[gtid >> 5] * 32u + (gtid & 31) : nullptr;
+    if (kCount) {                       // re-arm the scan of the list lengths that follows
+        if (gtid < (int)P.n_list_tiles) list_scan_tile[gtid] = 0ull;
+        if (gtid == 0) { *list_scan_ticket = 0u; list_cnt[P.n] = 0u; }
+    }
+    // fill mode: the NP's own list (list_start = exclusive scan of the padded lengths), written
+    // four entries (16 bytes) at a time
+    uint4 *col = kMode == 2 && gtid < P.n ? reinterpret_cast<uint4 *>(list + list_start[P.n - 1 - gtid]) : nullptr;
+    uint4 ebuf = make_uint4(0u, 0u, 0u, 0u);
     const float4 pi = pos[self];
     const int a = live ? __float_as_int(pi.w) : 0;
     const LvPair *pair_a = s_pair + a * LV_MAX_TYPES;
@@ -591,7 +601,14 @@ k_pair_force_s(const __grid_constant__ LvDev P, const float4 *__restrict__ pos,
                 const bool in = r2 < rc2 && jj[u] != self;           // fp32 contract #2
                 if (kList) {
                     if (in) {
-                        if (!kCount) col[(size_t)cnt * 32u] = jj[u];
+                        if (!kCount) {
+                            const int q = cnt & 3;
+                            ebuf.x = q == 0 ? jj[u] : ebuf.x;
+                            ebuf.y = q == 1 ? jj[u] : ebuf.y;
+                            ebuf.z = q == 2 ? jj[u] : ebuf.z;
+                            ebuf.w = jj[u];
+                            if (q == 3) col[cnt >> 2] = ebuf;
+                        }
                         ++cnt;
                     }
                     continue;
@@ -808,13 +825,21 @@ k_pair_force_s(const __grid_constant__ LvDev P, const float4 *__restrict__ pos,
         unpack2(fz2, lo, hi); fz = lo + hi;
     }
     if (kList) {
-        // rows of the tile = the longest column; shorter columns are filled with the lane's
-        // own slot, which the force kernel rejects by j != i
-        const int rows = __reduce_max_sync(kFull, cnt);
+        // lengths are padded to a multiple of 4 entries (16-byte stores and starts); the padding
+        // holds the NP's own slot, which the force kernel rejects by j != i
         if (kCount) {
-            if ((gtid & 31) == 0) list_rows[gtid >> 5] = (uint32_t)rows;
+            const uint32_t padded = live ? ((uint32_t)cnt + 3u) & ~3u : 0u;
+            if (live) list_cnt[i] = padded;
+            const uint32_t wsum = __reduce_add_sync(kFull, padded);
+            if ((gtid & 31) == 0 && wsum) atomicAdd(&st->list_total, (unsigned long long)wsum);
         } else {
-            for (int t = cnt; t < rows; ++t) col[(size_t)t * 32u] = self;
+            const int q = cnt & 3;              // the last, partial group: padded with the NP's own slot
+            if (live && q != 0) {
+                ebuf.y = q > 1 ? ebuf.y : self;
+                ebuf.z = q > 2 ? ebuf.z : self;
+                ebuf.w = self;
+                col[cnt >> 2] = ebuf;
+            }
             if (gtid == 0) st->n_rebuilds += 1u;
         }
         return;
@@ -822,82 +847,130 @@ k_pair_force_s(const __grid_constant__ LvDev P, const float4 *__restrict__ pos,
     if (live) force[i] = make_float4(fx, fy, fz, __int_as_float(cnt));
 }
 
-// Pair force from the skin neighbour list (lv_set_neighbour_list).  Lane = NP, as in the
-// build; the warp reads row t of its tile with ONE coalesced load (32 slot indices), each
-// lane gathers its candidate's position and evaluates contract #2 and the force -- no cell
-// arithmetic, no runs: the instruction stream is the distance test and the force.  The
-// positions are those of the list's slot order: posB on the step that rebuilt, else posA
+// Pair force from the skin neighbour list (lv_set_neighbour_list).  An NP's list is one
+// contiguous run of slot indices in walk order (ascending slots inside every stencil row), so
+// S lanes share ONE NP: they read S consecutive indices with one coalesced load and gather S
+// candidates that mostly sit in the same or neighbouring cache lines (the lane-per-NP tiles
+// of round 1 gathered from ~25 different lines per request); the S partial sums are added by
+// xor shuffles in a fixed order.  S is chosen on the device at every rebuild from the mean
+// list length (LvDevState::list_lanes: 4 below 64 entries, else 8; LV_OPT_LIST_LANES forces it).
+// The positions are those of the list's slot order: posB on the step that rebuilt, else posA
 // (k_update keeps that order until the next rebuild).
-constexpr int kLChunk = 4;
+constexpr int kRThreads = 128;
+constexpr int kRPerWarp = 8;        // NPs per warp: small work items, balanced by the block scheduler
+
+template <bool kCharged, int S>
+__device__ __forceinline__ void rows_body(const LvDev &P, const float4 *__restrict__ pos,
+                                          const uint32_t *__restrict__ list,
+                                          const uint32_t *__restrict__ list_start,
+                                          float4 *__restrict__ force, const LvPair *s_pair)
+{
+    constexpr int T = 32 / S;
+    constexpr int G = T > kRPerWarp ? T : kRPerWarp;    // NPs per warp
+    const int lane = threadIdx.x & 31;
+    const int ls = lane % S, lt = lane / S;             // sub-stream of the list, NP of the group
+    // the warp's consecutive sorted slots, from the END of the sorted order first, T at a time
+    // (the launch has a warp per kRPerWarp NPs; with G > kRPerWarp the surplus warps leave)
+    const int wbase = P.n - G * (int)(blockIdx.x * (kRThreads / 32) + (threadIdx.x >> 5) + 1);
+    if (wbase + G <= 0) return;
+#pragma unroll 1
+    for (int g0 = 0; g0 < G; g0 += T) {
+        const int i = wbase + g0 + lt;
+        const bool live = i >= 0;
+        const uint32_t self = live ? (uint32_t)i : 0u;
+        const float4 pi = pos[self];
+        const LvPair *pair_a = s_pair + (live ? __float_as_int(pi.w) : 0) * LV_MAX_TYPES;
+        const uint32_t b0 = live ? __ldg(list_start + i) : 0u;
+        const uint32_t len = live ? __ldg(list_start + i + 1) - b0 : 0u;     // a multiple of 4
+        const uint32_t maxlen = __reduce_max_sync(kFull, len);
+        const uint32_t *lp = list + b0 + ls;
+        float fx = 0.f, fy = 0.f, fz = 0.f;
+        int cnt = 0;
+        // Gather u of a round takes the S CONSECUTIVE entries u S .. u S + S - 1 of every NP of
+        // the group (ascending slots: few cache lines per request).  Software pipeline: the
+        // indices of the next round are loading while this one is evaluated.
+        uint32_t jn[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) jn[u] = (uint32_t)(u * S + ls) < len ? __ldg(lp + u * S) : self;
+        for (uint32_t k0 = 0; k0 < maxlen; k0 += 4u * S) {
+            uint32_t jj[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) jj[u] = jn[u];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const uint32_t kn = k0 + (uint32_t)((4 + u) * S + ls);
+                jn[u] = kn < len ? __ldg(lp + (k0 + (uint32_t)((4 + u) * S))) : self;
+            }
+            float4 pj[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) pj[u] = __ldg(pos + jj[u]);
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const LvPair pr = pair_a[__float_as_int(pj[u].w)];
+                const float dx = __fsub_rn(pi.x, pj[u].x);
+                const float dy = __fsub_rn(pi.y, pj[u].y);
+                const float dz = __fsub_rn(pi.z, pj[u].z);
+                const float r2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
+                const bool in = r2 < pr.rc2 && jj[u] != self;            // fp32 contract #2
+                const float rinv = rsqrt_approx(r2);
+                const float ir2 = rinv * rinv;
+                const float ir6 = ir2 * ir2 * ir2;
+                float f = fmaf(pr.c12, ir6, -pr.c6) * ir6;
+                if (kCharged) f = fmaf(pr.qq, rinv, f);
+                f *= ir2;
+                f = in ? f : 0.0f;
+                fx = fmaf(f, dx, fx);
+                fy = fmaf(f, dy, fy);
+                fz = fmaf(f, dz, fz);
+                cnt += in ? 1 : 0;
+            }
+        }
+#pragma unroll
+        for (int d = 1; d < S; d <<= 1) {
+            fx += __shfl_xor_sync(kFull, fx, d);
+            fy += __shfl_xor_sync(kFull, fy, d);
+            fz += __shfl_xor_sync(kFull, fz, d);
+            cnt += __shfl_xor_sync(kFull, cnt, d);
+        }
+        if (live && ls == 0) force[i] = make_float4(fx, fy, fz, __int_as_float(cnt));
+    }
+}
 
 template <bool kCharged>
-__global__ void __launch_bounds__(kSThreads)
-k_pair_force_list(const __grid_constant__ LvDev P, const float4 *__restrict__ posA,
+__global__ void __launch_bounds__(kRThreads)
+k_pair_force_rows(const __grid_constant__ LvDev P, const float4 *__restrict__ posA,
                   const float4 *__restrict__ posB, const uint32_t *__restrict__ list,
-                  const uint32_t *__restrict__ list_rows, const uint32_t *__restrict__ list_off,
-                  float4 *__restrict__ force, const LvDevState *st)
+                  const uint32_t *__restrict__ list_start, float4 *__restrict__ force,
+                  const LvDevState *st)
 {
     if (st->list_ok == 0u) return;          // the cell kernel takes this step
     __shared__ LvPair s_pair[LV_MAX_TYPES * LV_MAX_TYPES];
-    for (int t = threadIdx.x; t < LV_MAX_TYPES * LV_MAX_TYPES; t += kSThreads) s_pair[t] = P.pair[t];
+    for (int t = threadIdx.x; t < LV_MAX_TYPES * LV_MAX_TYPES; t += kRThreads) s_pair[t] = P.pair[t];
     __syncthreads();
     const float4 *__restrict__ pos = st->rebuild[st->step & 1] ? posB : posA;
-    const int gtid = (int)(blockIdx.x * kSThreads + threadIdx.x);
-    const int i = P.n - 1 - gtid;
-    const bool live = i >= 0;
-    const uint32_t self = live ? (uint32_t)i : 0u;
-    const float4 pi = pos[self];
-    const LvPair *pair_a = s_pair + (live ? __float_as_int(pi.w) : 0) * LV_MAX_TYPES;
-    const uint32_t *col = list + (size_t)list_off[gtid >> 5] * 32u + (gtid & 31);
-    const int rows = (int)list_rows[gtid >> 5];
-    float fx = 0.f, fy = 0.f, fz = 0.f;
-    int cnt = 0;
+    const unsigned int S = P.list_lanes_forced ? (unsigned int)P.list_lanes_forced : st->list_lanes;
+    if (S == 1u) rows_body<kCharged, 1>(P, pos, list, list_start, force, s_pair);
+    else if (S == 2u) rows_body<kCharged, 2>(P, pos, list, list_start, force, s_pair);
+    else if (S == 4u) rows_body<kCharged, 4>(P, pos, list, list_start, force, s_pair);
+    else if (S == 8u) rows_body<kCharged, 8>(P, pos, list, list_start, force, s_pair);
+    else if (S == 16u) rows_body<kCharged, 16>(P, pos, list, list_start, force, s_pair);
+    else rows_body<kCharged, 32>(P, pos, list, list_start, force, s_pair);
+}
 
-    // three chunks in flight: the slot indices of chunk c + 2 and the positions of chunk
-    // c + 1 are loading while chunk c is evaluated (the gather is a dependent load pair)
-    auto fetch_idx = [&](int t, uint32_t (&jj)[kLChunk]) {
-#pragma unroll
-        for (int u = 0; u < kLChunk; ++u) jj[u] = t + u < rows ? __ldg(col + (size_t)(t + u) * 32u) : self;
-    };
-    auto fetch_pos = [&](const uint32_t (&jj)[kLChunk], float4 (&pj)[kLChunk]) {
-#pragma unroll
-        for (int u = 0; u < kLChunk; ++u) pj[u] = __ldg(pos + jj[u]);
-    };
-    auto eval = [&](const uint32_t (&jj)[kLChunk], const float4 (&pj)[kLChunk]) {
-#pragma unroll
-        for (int u = 0; u < kLChunk; ++u) {
-            const LvPair pr = pair_a[__float_as_int(pj[u].w)];
-            const float dx = __fsub_rn(pi.x, pj[u].x);
-            const float dy = __fsub_rn(pi.y, pj[u].y);
-            const float dz = __fsub_rn(pi.z, pj[u].z);
-            const float r2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
-            const bool in = r2 < pr.rc2 && jj[u] != self;            // fp32 contract #2
-            const float rinv = rsqrt_approx(r2);
-            const float ir2 = rinv * rinv;
-            const float ir6 = ir2 * ir2 * ir2;
-            float f = fmaf(pr.c12, ir6, -pr.c6) * ir6;
-            if (kCharged) f = fmaf(pr.qq, rinv, f);
-            f *= ir2;
-            f = in ? f : 0.0f;
-            fx = fmaf(f, dx, fx);
-            fy = fmaf(f, dy, fy);
-            fz = fmaf(f, dz, fz);
-            cnt += in ? 1 : 0;
-        }
-    };
-    uint32_t ja[kLChunk], jb[kLChunk], jc[kLChunk];
-    float4 pa[kLChunk], pb[kLChunk], pc[kLChunk];
-    fetch_idx(0, ja);
-    fetch_idx(kLChunk, jb);
-    fetch_pos(ja, pa);
-    for (int t = 0; t < rows; t += 3 * kLChunk) {
-        fetch_idx(t + 2 * kLChunk, jc); fetch_pos(jb, pb); eval(ja, pa);
-        if (t + kLChunk >= rows) break;
-        fetch_idx(t + 3 * kLChunk, ja); fetch_pos(jc, pc); eval(jb, pb);
-        if (t + 2 * kLChunk >= rows) break;
-        fetch_idx(t + 4 * kLChunk, jb); fetch_pos(ja, pa); eval(jc, pc);
-    }
-    if (live) force[i] = make_float4(fx, fy, fz, __int_as_float(cnt));
+// After the count pass and the scan of the lengths: does the list fit its pool, and how many
+// lanes share an NP's list (from the mean length, so the choice is a function of the state).
+__global__ void k_list_check(int n, uint32_t pool, LvDevState *st)
+{
+    if (skipped(st)) return;
+    if (st->list_ok == 0u && (st->step & 63) != 0) return;       // not counted this step
+    const unsigned long long total = st->list_total;
+    const bool fits = total <= (unsigned long long)pool;
+    st->list_ok = fits ? 1u : 0u;
+    st->list_used = total;
+    st->list_total = 0ull;
+    const unsigned long long mean = total / (unsigned long long)(n > 0 ? n : 1);
+    st->list_lanes = mean < 64ull ? 4u : 8u;          // measured on C3
+    if (!fits) atomicOr(&st->status, LV_ST_LIST_OVERFLOW);
 }
 
 // ------------------------------------------------- A1 + A7 fused update
@@ -1057,7 +1130,9 @@ k_pack_state(int n, int n_types, const float *__restrict__ pos, const float *__r
         st->rebuild[(step + 1) & 1] = 0u;
         st->n_rebuilds = 0u;
         st->list_ok = 1u;
-        st->list_rows_used = 0u;
+        st->list_lanes = 32u;
+        st->list_total = 0ull;
+        st->list_used = 0ull;
         st->n_fallback = 0u;
     }
     if (i >= n) return;
@@ -1553,81 +1628,49 @@ cudaError_t lvk_pair_force(const LvDev &P, const LvBufs &B, int variant, cudaStr
         if (variant == 3) {
             if (charged)
                 k_pair_force_s<true, 1><<<blocks, kSThreads, 0, st>>>(P, B.posB, B.cell_off, B.force,
-                                                                      B.posP, nullptr, nullptr, nullptr, nullptr);
+                                                                      B.posP, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr);
             else
                 k_pair_force_s<false, 1><<<blocks, kSThreads, 0, st>>>(P, B.posB, B.cell_off, B.force,
-                                                                       B.posP, nullptr, nullptr, nullptr, nullptr);
+                                                                       B.posP, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr);
         } else {
             if (charged)
                 k_pair_force_s<true, 0><<<blocks, kSThreads, 0, st>>>(P, B.posB, B.cell_off, B.force,
-                                                                      nullptr, nullptr, nullptr, nullptr, nullptr);
+                                                                      nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr);
             else
                 k_pair_force_s<false, 0><<<blocks, kSThreads, 0, st>>>(P, B.posB, B.cell_off, B.force,
-                                                                       nullptr, nullptr, nullptr, nullptr, nullptr);
+                                                                       nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr);
         }
     }
     return cudaGetLastError();
 }
 
-// Exclusive scan of the rows per warp -> tile offsets; decides whether the list fits its pool
-// (one block: the table has n / 32 entries).
-namespace {
-constexpr int kLScanThreads = 1024;
-__global__ void __launch_bounds__(kLScanThreads)
-k_list_scan(int n_warps, uint32_t pool_rows, const uint32_t *__restrict__ rows, uint32_t *__restrict__ offs,
-            LvDevState *st)
-{
-    if (skipped(st)) return;
-    if (st->list_ok == 0u && (st->step & 63) != 0) return;       // not counted this step
-    __shared__ unsigned long long s_sum[kLScanThreads];
-    const int per = (n_warps + kLScanThreads - 1) / kLScanThreads;
-    const int lo = threadIdx.x * per, hi = min(lo + per, n_warps);
-    unsigned long long sum = 0ull;
-    for (int k = lo; k < hi; ++k) sum += rows[k];
-    s_sum[threadIdx.x] = sum;
-    __syncthreads();
-    for (int d = 1; d < kLScanThreads; d <<= 1) {                 // inclusive scan of the chunk sums
-        const unsigned long long v = threadIdx.x >= d ? s_sum[threadIdx.x - d] : 0ull;
-        __syncthreads();
-        s_sum[threadIdx.x] += v;
-        __syncthreads();
-    }
-    const unsigned long long total = s_sum[kLScanThreads - 1];
-    const bool fits = total <= (unsigned long long)pool_rows;
-    if (fits) {
-        unsigned long long run = s_sum[threadIdx.x] - sum;
-        for (int k = lo; k < hi; ++k) { offs[k] = (uint32_t)run; run += rows[k]; }
-    }
-    if (threadIdx.x == 0) {
-        st->list_ok = fits ? 1u : 0u;
-        st->list_rows_used = total > 0xffffffffull ? 0xffffffffu : (uint32_t)total;
-        if (!fits) atomicOr(&st->status, LV_ST_LIST_OVERFLOW);
-    }
-}
-}  // namespace
-
-// skin list: tiles are indexed by the launch's warp id, so count, fill and force use the same grid
+// skin list: count the (padded) list lengths, scan them into the list starts, check the pool,
+// fill -- all guarded by this step's rebuild flag
 cudaError_t lvk_list_build(const LvDev &P, const LvBufs &B, cudaStream_t st)
 {
-    const int blocks = (P.n + kSThreads - 1) / kSThreads;
+    const int m = P.n > (int)P.n_list_tiles ? P.n : (int)P.n_list_tiles;
+    const int blocks = (m + kSThreads - 1) / kSThreads;
     k_pair_force_s<false, 3><<<blocks, kSThreads, 0, st>>>(P, B.posB, B.cell_off, nullptr, nullptr, nullptr,
-                                                           B.list_rows, nullptr, B.st);
-    k_list_scan<<<1, kLScanThreads, 0, st>>>(blocks * (kSThreads / 32), P.list_pool_rows, B.list_rows,
-                                             B.list_off, B.st);
-    k_pair_force_s<false, 2><<<blocks, kSThreads, 0, st>>>(P, B.posB, B.cell_off, nullptr, nullptr, B.list,
-                                                           B.list_rows, B.list_off, B.st);
+                                                           B.list_cnt, nullptr, B.list_scan_tile,
+                                                           B.list_scan_ticket, B.st);
+    k_scan_cells<<<P.n_list_tiles, kScanThreads, 0, st>>>((uint32_t)P.n + 1u, B.list_cnt, B.list_start,
+                                                          B.list_scan_tile, B.list_scan_ticket, B.st, B.st);
+    k_list_check<<<1, 1, 0, st>>>(P.n, P.list_pool, B.st);
+    k_pair_force_s<false, 2><<<(P.n + kSThreads - 1) / kSThreads, kSThreads, 0, st>>>(
+        P, B.posB, B.cell_off, nullptr, nullptr, B.list, nullptr, B.list_start, nullptr, nullptr, B.st);
     return cudaGetLastError();
 }
 
 cudaError_t lvk_pair_force_list(const LvDev &P, const LvBufs &B, cudaStream_t st)
 {
-    const int blocks = (P.n + kSThreads - 1) / kSThreads;
+    const int per_block = kRPerWarp * (kRThreads / 32);
+    const int blocks = (P.n + per_block - 1) / per_block;
     if (lvk_any_charge(P))
-        k_pair_force_list<true><<<blocks, kSThreads, 0, st>>>(P, B.posA, B.posB, B.list, B.list_rows,
-                                                              B.list_off, B.force, B.st);
+        k_pair_force_rows<true><<<blocks, kRThreads, 0, st>>>(P, B.posA, B.posB, B.list, B.list_start,
+                                                              B.force, B.st);
     else
-        k_pair_force_list<false><<<blocks, kSThreads, 0, st>>>(P, B.posA, B.posB, B.list, B.list_rows,
-                                                               B.list_off, B.force, B.st);
+        k_pair_force_rows<false><<<blocks, kRThreads, 0, st>>>(P, B.posA, B.posB, B.list, B.list_start,
+                                                               B.force, B.st);
     return cudaGetLastError();
 }
 
@@ -1636,10 +1679,10 @@ cudaError_t lvk_pair_force_fallback(const LvDev &P, const LvBufs &B, cudaStream_
     const int blocks = (P.n + kSThreads - 1) / kSThreads;
     if (lvk_any_charge(P))
         k_pair_force_s<true, 0><<<blocks, kSThreads, 0, st>>>(P, B.posB, B.cell_off, B.force, nullptr, nullptr,
-                                                              nullptr, nullptr, B.st);
+                                                              nullptr, nullptr, nullptr, nullptr, B.st);
     else
         k_pair_force_s<false, 0><<<blocks, kSThreads, 0, st>>>(P, B.posB, B.cell_off, B.force, nullptr, nullptr,
-                                                               nullptr, nullptr, B.st);
+                                                               nullptr, nullptr, nullptr, nullptr, B.st);
     return cudaGetLastError();
 }
 
@@ -1656,7 +1699,7 @@ cudaError_t lvk_scan_cells(const LvDev &P, const LvBufs &B, bool guarded, cudaSt
 {
     k_scan_cells<<<P.n_scan_tiles, kScanThreads, 0, st>>>(P.n_cells + 1u, B.cell_cnt, B.cell_off,
                                                           B.scan_tile, B.scan_ticket,
-                                                          guarded ? B.st : nullptr);
+                                                          guarded ? B.st : nullptr, nullptr);
     return cudaGetLastError();
 }
 
