@@ -60,7 +60,45 @@ FLUSH_BYTES = 256 << 20            # > 126 MB L2
 # accumulation = 22.  Charged pairs add 4 (rsqrt, mul, fma); not counted here,
 # so the figure is a lower bound.
 FLOP_PER_PAIR = 22.0
+# "algorithmic flops = the in-range ordered pairs x ~33 (distance test +
+# force)".  roofline.frac uses THIS figure and the FMA peak measured in the same run; the
+# 22-flop count and the nominal peak are kept as secondary keys.
+FLOP_PER_PAIR_SURVEY = 33.0
 FP32_LANES_PER_SM = 128
+KERNEL_OF_PATH = {"list": "k_pair_force_rows", "cells": "k_pair_force_s", "tile": "k_pair_force_t",
+                  "packed": "k_pair_force_s", "queued": "k_pair_force_q", "simple": "k_pair_force"}
+
+
+def source_hash():
+    """Content hash of the CUDA sources + the header: ncu figures are only quoted for the
+    kernels they were captured on."""
+    import hashlib
+    h = hashlib.sha256()
+    base = os.path.join(ROOT, "paper_2501_04456_b200", "csrc")
+    for f in sorted(os.listdir(base)):
+        with open(os.path.join(base, f), "rb") as fh:
+            h.update(f.encode() + b"\0" + fh.read())
+    with open(os.path.join(ROOT, "include", "lv.h"), "rb") as fh:
+        h.update(fh.read())
+    return h.hexdigest()[:16]
+
+
+def ncu_record(kernel, workload, start_step, path):
+    """The entry of profiles/ncu_kernels.json (written by `python -m paper_2501_04456_b200.ncu_summary`
+    from a committed ncu command) for this kernel / workload / step / force path, or None.
+    `stale` says whether the sources have changed since the capture."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "ncu_kernels.json")) as f:
+            recs = json.load(f)
+    except Exception:
+        return None
+    for r in recs:
+        if (r.get("kernel") == kernel and r.get("workload") == workload
+                and int(r.get("start_step", -1)) == int(start_step) and r.get("path") == path):
+            r = dict(r)
+            r["stale"] = r.get("source_hash") != source_hash()
+            return r
+    return None
 
 
 def peaks():
@@ -168,19 +206,58 @@ def timed_steps_product(sim, torch, flush, k):
 
 
 def inrange_pairs(sim):
+    """In-range ordered pairs of the current state (lv_compute_forces: always the cells, does
+    not disturb a list run)."""
     sim.compute_forces()
     _, cnt = sim.get_forces()
     return float(cnt.astype(np.int64).sum())
 
 
-def measure_point(sim, torch, flush, w, steps, warmup):
-    """One measurement of the resident-state throughput at the current step."""
+def force_path_of(args):
+    if args.force_kernel in (None, 2):
+        return "cells" if args.no_list else "list"
+    return {0: "simple", 1: "queued", 3: "packed", 4: "tile"}[args.force_kernel]
+
+
+def make_sim(binding, w, args, device, cpc=None, use_list=None):
+    """The product path: the workload's tuned grids and -- unless --no-list -- the automatic
+    skin neighbour list (lv_set_neighbour_list(skin <= 0, -1))."""
+    options = {}
+    if args.force_kernel is not None:
+        options[binding.OPT_FORCE_KERNEL] = args.force_kernel
+    if args.tile_substreams is not None:
+        options[binding.OPT_TILE_SUBSTREAMS] = args.tile_substreams
+    if cpc is None:
+        cpc = args.cells_per_cut if args.cells_per_cut else w.tuned_cells_per_cut
+    if use_list is None:
+        use_list = not args.no_list and args.force_kernel in (None, 2)
+    nl = (args.skin, -1) if use_list else None
+    return binding.Simulation.from_workload(w, cells_per_cut=cpc, device=device, options=options or None,
+                                            neighbour_list=nl), cpc, use_list
+
+
+def measure_point(sim, torch, flush, n, steps, warmup, peak_tflops):
+    """Flushed product-path time of `steps` steps from the current state, then the stage pass
+    over the next `steps` steps and the roofline figures of the pair-force stage."""
     timed_steps_product(sim, torch, flush, max(warmup, 1))
     tot = timed_steps_product(sim, torch, flush, steps)
     p0 = inrange_pairs(sim)
-    stages, _ = timed_steps(sim, torch, flush, steps)
+    stages, stot = timed_steps(sim, torch, flush, steps)
     p1 = inrange_pairs(sim)
-    return stages, tot, 0.5 * (p0 + p1)
+    pairs = 0.5 * (p0 + p1)
+    fm = stages["pair_force"] / steps
+    return {"ms_per_step": tot / steps, "value": float(n) * steps / (tot * 1e-3), "unit": UNIT,
+            "stage_ms_per_step": {k: v / steps for k, v in stages.items()},
+            "kernel_ms": fm, "in_range_ordered_pairs": pairs,
+            "frac": FLOP_PER_PAIR_SURVEY * pairs / (fm * 1e-3) * 1e-12 / peak_tflops if fm > 0 else None}
+
+
+def list_info(sim, use_list):
+    if not use_list:
+        return None
+    st = sim.list_stats()
+    return {"rebuilds": st["rebuilds"], "fallback_steps": st["fallback_steps"],
+            "entries_used": st["entries_used"], "pool_entries": st["pool_entries"]}
 
 
 def run_lv(args):
@@ -200,24 +277,25 @@ def run_lv(args):
         replicas.init("nccl")
     binding.load()
     pk = peaks()
+    solo = rank == 0 and world == 1
 
     base = workloads.make_workload(args.workload, state=False)
     w = workloads.make_workload(args.workload, seed=replicas.replica_seed(base.seed, rank))
-    options = None if args.force_kernel is None else {binding.OPT_FORCE_KERNEL: args.force_kernel}
-    cpc = args.cells_per_cut if args.cells_per_cut else w.tuned_cells_per_cut
-    nl = None if args.neighbour_list is None else (args.neighbour_list[0], int(args.neighbour_list[1]))
-    sim = binding.Simulation.from_workload(w, cells_per_cut=cpc, device=device, options=options,
-                                           neighbour_list=nl)
+    n = w.n
+    sim, cpc, use_list = make_sim(binding, w, args, device)
+    path = force_path_of(args)
     if args.start_step > 0:
         sim.step(args.start_step)
         sim.get_state()                      # synchronises; raises on a non-finite state
     flush = torch.empty(FLUSH_BYTES, dtype=torch.uint8, device=device)
     n_sms = torch.cuda.get_device_properties(device).multi_processor_count
-    fma_tflops = sim.measure_fp32_peak()
+    fma_tflops = sim.measure_fp32_peak()     # the roofline's denominator: measured in this run
+    nominal_tflops = n_sms * FP32_LANES_PER_SM * 2 * pk["sm_max_mhz"] * 1e6 * 1e-12
 
     # ---- timed region: K steps of the product path (graph replay), events on the
     # library's stream around every step --------------------------------------
     timed_steps_product(sim, torch, flush, max(args.warmup, 3))
+    l0 = list_info(sim, use_list)
     sampler = ClockSampler(visible_gpu_index(local_rank))
     replicas.barrier()
     torch.cuda.synchronize()
@@ -228,6 +306,7 @@ def run_lv(args):
     wall_s = time.perf_counter() - t_wall0
     clocks = sampler.finish()
     replicas.barrier()
+    l1 = list_info(sim, use_list)
     # ---- stage pass: the next K steps launched kernel by kernel with an event after every
     # stage (lv_stage_timing); the event records cost ~2.5 us per stage, so this pass is
     # the breakdown and the source of the pair-force kernel time, not the headline
@@ -236,60 +315,47 @@ def run_lv(args):
     pairs1 = inrange_pairs(sim)
     launches_per_step = sim.launches_per_step()
 
-    ms_max, units = replicas.reduce_timing(tot_ms, float(w.n) * args.steps, device=device)
+    ms_max, units = replicas.reduce_timing(tot_ms, float(n) * args.steps, device=device)
     value = units / (ms_max * 1e-3)
 
-    # ---- the same K steps as one graph replay, state L2-resident -----------
+    # ---- a longer window without flushes: lv_step(K') as graph replays, the state (and, at this
+    # size, the list) L2-resident -- how a simulation actually runs; K' >= 500 so that the
+    # rebuilds of the list are averaged over
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    kres = max(args.steps, args.resident_steps)
     sim.step(max(args.warmup, 3))
     sim.synchronize()
+    l2 = list_info(sim, use_list)
     e0.record(sim.stream)
-    sim.step(args.steps)
+    sim.step(kres)
     e1.record(sim.stream)
     e1.synchronize()
     res_ms = e0.elapsed_time(e1)
+    l3 = list_info(sim, use_list)
     res_max, _ = replicas.reduce_timing(res_ms, 0.0, device=device)
 
-    # ---- variant (not the headline): persistent skin neighbour list, NEXT-3 -
+    # ---- variant (not the headline): the paper's literal scheme, cells rebuilt every step ----
     variants = {}
-    if (rank == 0 and world == 1 and nl is None and not args.no_variants
-            and w.tuned_neighbour_list is not None):
-        skin, cap = float(w.tuned_neighbour_list[0]), int(w.tuned_neighbour_list[1])
-        vs = binding.Simulation.from_workload(w, cells_per_cut=cpc, device=device,
-                                              neighbour_list=(skin, cap))
+    if solo and use_list and not args.no_variants:
+        vs, _, _ = make_sim(binding, w, args, device, cpc=cpc, use_list=False)
         if args.start_step > 0:
             vs.step(args.start_step)
-        timed_steps_product(vs, torch, flush, max(args.warmup, 3))
-        r0 = vs.rebuild_count()
-        vtot = timed_steps_product(vs, torch, flush, args.steps)
-        r1 = vs.rebuild_count()
-        vstages, _ = timed_steps(vs, torch, flush, args.steps)
+        v = measure_point(vs, torch, flush, n, args.steps, max(args.warmup, 3), fma_tflops)
         vs.step(max(args.warmup, 3))
         vs.synchronize()
         e0.record(vs.stream)
-        vs.step(args.steps)
+        vs.step(kres)
         e1.record(vs.stream)
         e1.synchronize()
-        vres = e0.elapsed_time(e1)
-        vs.get_state()                       # raises if the list overflowed
-        variants["skin_list"] = {
-            "what": "lv_set_neighbour_list: cells + list rebuilt on the device only when an NP has "
-                    "moved skin/2; same neighbour counts, forces to rounding (tests/test_gpu_neighbour_list.py)",
-            "skin": skin, "capacity": cap,
-            "value": float(w.n) * args.steps / (vtot * 1e-3), "unit": UNIT,
-            "ms_per_step": vtot / args.steps,
-            "stage_ms_per_step": {k: v / args.steps for k, v in vstages.items()},
-            "rebuilds_in_timed_region": r1 - r0,
-            "resident_ms_per_step": vres / args.steps,
-            "pair_force_roofline_frac": FLOP_PER_PAIR * 0.5 * (pairs0 + pairs1)
-            / (vstages["pair_force"] / args.steps * 1e-3) * 1e-12
-            / (n_sms * FP32_LANES_PER_SM * 2 * pk["sm_max_mhz"] * 1e6 * 1e-12),
-        }
+        v["resident_ms_per_step"] = e0.elapsed_time(e1) / kres
+        v["what"] = ("lv_set_neighbour_list off: cell hash, sort, offsets and the cell-walk force kernel "
+                     "(k_pair_force_s) every step, as PAPER.md:62-69 does")
+        variants["cells_every_step"] = v
         vs.close()
 
     # ---- variant: many small droplets at once (NEXT-3 batched replicas; the paper's own
     # sizes, Table 1: 10^4 NPs, fill a fraction of a B200) -- R handles on R streams
-    if rank == 0 and world == 1 and not args.no_variants and args.small_replicas > 0:
+    if solo and not args.no_variants and args.small_replicas > 0:
         ks = 1000
         sr = {}
         for R_ in (1, args.small_replicas):
@@ -317,7 +383,7 @@ def run_lv(args):
 
     # ---- NEXT-1 rows: the paper's observables on the device (synchronous calls) -------
     observables = {}
-    if rank == 0 and world == 1 and not args.no_variants:
+    if solo and not args.no_variants:
         nb = 100
         drb = 5.0 / nb                                  # g(r) to r = 5 sigma, as in the long-run tests
         sim.observe_rdf(drb, nb); sim.observe_radial(w.R0 / 100.0, 128)      # warm
@@ -355,7 +421,6 @@ def run_lv(args):
         }
 
     # ---- e2e: host buffers through the C ABI, copies inside the timed region
-    n = w.n
     hp = torch.empty((n, 3), dtype=torch.float32).pin_memory()
     hv = torch.empty((n, 3), dtype=torch.float32).pin_memory()
     ht = torch.empty((n,), dtype=torch.int32).pin_memory()
@@ -385,30 +450,29 @@ def run_lv(args):
     # ---- roofline of the dominant kernel (pair force) ----------------------
     force_ms = stages["pair_force"] / args.steps
     pairs = 0.5 * (pairs0 + pairs1)
-    flops = FLOP_PER_PAIR * pairs
-    peak_tflops = n_sms * FP32_LANES_PER_SM * 2 * pk["sm_max_mhz"] * 1e6 * 1e-12
-    achieved = flops / (force_ms * 1e-3) * 1e-12
+    kernel = KERNEL_OF_PATH[path]
+    achieved = FLOP_PER_PAIR_SURVEY * pairs / (force_ms * 1e-3) * 1e-12
+    rec = ncu_record(kernel, w.name, args.start_step, path)
+    usable = rec is not None and not rec["stale"]
     roofline = {
-        "kernel": "k_pair_force_s" if args.force_kernel in (None, 2, 3) else "k_pair_force", "bound": "alu",
-        "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s",
-        "frac": achieved / peak_tflops,
-        # dram__bytes_read.sum + dram__bytes_write.sum of k_pair_force_s per launch from the committed
-        # ncu --set full capture of this command (profiles/r1c_segments_C3.md: 6.90 MB read, 0 written);
-        # only meaningful for the default kernel and workload it was captured on
-        "traffic": args.force_traffic_bytes if args.force_traffic_bytes is not None else (
-            6.8965e6 if (w.name == "C3" and args.force_kernel in (None, 2) and args.start_step == 0
-                         and nl is None) else None),
-        "traffic_source": "profiles/r1c_segments_C3.md (ncu --set full, cold cache); algorithmic 32 B/NP = "
-                          f"{32 * n} B",
-        "executed_fp32_util_ncu": "21 % of FP32-lane slots at step 0, 31 % at step 17 000 "
-                                  "(profiles/r1c_segments_C3.md, r1d_dense_states_C3.md)",
-        "peak_source": f"{n_sms} SMs x 128 FP32 lanes x 2 x {pk['sm_max_mhz']:.0f} MHz "
-                       f"(DESIGN.md); measured FMA microkernel {fma_tflops:.1f} TFLOP/s",
-        "algorithmic_flops_per_launch": flops,
-        "in_range_ordered_pairs": pairs, "flop_per_pair": FLOP_PER_PAIR,
-        # SURVEY 8(d) quotes "~33" flops per in-range pair (distance test + force); DESIGN.md sec. 7
-        # counts 22 (Coulomb's 4 not counted).  The fraction at the survey's figure, for comparison:
-        "frac_at_33_flop_per_pair": 33.0 / FLOP_PER_PAIR * achieved / peak_tflops,
+        "kernel": kernel, "bound": "alu",
+        "achieved": achieved, "peak": fma_tflops, "unit": "TFLOP/s",
+        "frac": achieved / fma_tflops,
+        "flop_per_pair": FLOP_PER_PAIR_SURVEY,
+        "peak_source": "FMA microkernel of this run (lv_measure_fp32_peak): %.1f TFLOP/s; nominal %d SMs x 128 "
+                       "FP32 lanes x 2 x %.0f MHz = %.1f TFLOP/s" % (fma_tflops, n_sms, pk["sm_max_mhz"], nominal_tflops),
+        "algorithmic_flops_per_launch": FLOP_PER_PAIR_SURVEY * pairs,
+        "in_range_ordered_pairs": pairs,
+        # secondary conventions: DESIGN.md's own count of 22 flop per pair, and the nominal peak
+        "frac_at_22_flop_per_pair": FLOP_PER_PAIR * pairs / (force_ms * 1e-3) * 1e-12 / fma_tflops,
+        "frac_of_nominal_peak": achieved / nominal_tflops,
+        # from the committed ncu capture of this kernel on this workload / step / path
+        # (profiles/ncu_kernels.json); null when there is none or the sources have changed since
+        "traffic": rec["dram_bytes"] if usable else None,
+        "executed_fp32_frac": rec["executed_fp32_frac"] if usable else None,
+        "ncu": ({"report": rec["report"], "duration_us": rec["duration_us"], "issue_active_pct": rec["issue_active_pct"],
+                 "l1_data_pipe_pct": rec["l1_data_pipe_pct"], "lts_bytes": rec["lts_bytes"],
+                 "source_hash": rec["source_hash"], "stale": rec["stale"]} if rec is not None else None),
         "kernel_ms": force_ms,
         "share_of_step": stages["pair_force"] / tot_ms,          # against the graph-replayed (headline) step
         "share_of_stage_pass": stages["pair_force"] / stage_tot_ms,   # that pass carries event overhead
@@ -422,35 +486,41 @@ def run_lv(args):
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms_max / args.steps, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-        "config": {"workload": f"{w.name} (BASELINE.json configs[{int(w.name[1]) - 1}]): N={n}, "
-                               f"{w.n_types} types, steps {args.start_step + 0}.. of the schedule",
-                   "n_particles": n, "start_step": args.start_step,
-                   "cells_per_cut": list(cpc) if cpc else [1] * w.n_types,
-                   "force_kernel": {0: "simple", 1: "queued", 2: "segments", 3: "packed"}[
-                       2 if args.force_kernel is None else args.force_kernel],
-                   "replicas": world, "parallelism": "independent replicas, no collective",
-                   "l2": "flushed between timed steps (256 MiB memset on the same stream)",
-                   "timing": "lv_step(1) = one CUDA-graph replay per step; a CUDA event pair on the library's stream around every step (the flush outside it); sum over K"},
+        "config": config_of(w, args.start_step, extra={
+            "cells_per_cut": list(cpc) if cpc else [1] * w.n_types,
+            "force_path": path, "force_kernel": kernel,
+            "neighbour_list": ("automatic skin and pool (lv_set_neighbour_list(<= 0, -1)): cells + list rebuilt on the "
+                               "device when an NP has moved skin/2, cell kernel when the pool is too small")
+            if use_list else "off: cells rebuilt every step",
+            "replicas": world, "parallelism": "independent replicas, no collective",
+            "l2": "flushed between timed steps (256 MiB memset on the same stream)",
+            "timing": "lv_step(1) = one CUDA-graph replay per step; a CUDA event pair on the library's stream "
+                      "around every step (the flush outside it); sum over K"}),
         "clocks": clocks,
         "gpu_launches": launches_per_step * args.steps,
         "launches_per_step": launches_per_step,
+        "list": ({"rebuilds_in_timed_region": l1["rebuilds"] - l0["rebuilds"],
+                  "fallback_steps_in_timed_region": l1["fallback_steps"] - l0["fallback_steps"],
+                  "entries_used": l1["entries_used"], "pool_entries": l1["pool_entries"]} if use_list else None),
         "stage_ms_per_step": {k: v / args.steps for k, v in stages.items()},
         "stage_pass_ms_per_step": stage_tot_ms / args.steps,
         "wall_s_timed_region": wall_s,
         "roofline": roofline,
         "variants": variants,
         "observables": observables,
-        "resident": {"value": float(n) * args.steps * world / (res_max * 1e-3), "unit": UNIT,
-                     "ms_per_step": res_max / args.steps,
-                     "how": "lv_step(K) as CUDA-graph replay, no L2 flush, events around the K steps"},
+        "resident": {"value": float(n) * kres * world / (res_max * 1e-3), "unit": UNIT,
+                     "ms_per_step": res_max / kres, "steps": kres,
+                     "rebuilds": (l3["rebuilds"] - l2["rebuilds"]) if use_list else None,
+                     "how": "lv_step(K') as CUDA-graph replays, no L2 flush, events around the K' steps"},
         "e2e": {"value": e2e_units / (e2e_max * 1e-3), "unit": UNIT, "steps": ke,
                 "h2d_bytes_per_step": 28 * n, "d2h_bytes_per_step": 28 * n + 16,
                 "ms_per_step": e2e_max / ke,
-                "how": "lv_set_state(host pinned) + lv_step(1) + lv_get_state(host pinned) per step"},
+                "how": "lv_set_state(host pinned) + lv_step(1) + lv_get_state(host pinned) per step "
+                       "(the first step after lv_set_state runs on the cell kernel: no list is built for one step)"},
     }
 
     # ---- further points of the schedule (not the headline) -----------------
-    if rank == 0 and world == 1 and args.snapshots:
+    if solo and args.snapshots:
         snaps = []
         for target in args.snapshots:
             _, _, _, _, cur = sim.get_state()
@@ -458,21 +528,61 @@ def run_lv(args):
                 continue
             sim.step(target - cur)
             _, _, _, Rn, cur = sim.get_state()
-            sg, tt, pp = measure_point(sim, torch, flush, w, args.snapshot_steps, 10)
-            fm = sg["pair_force"] / args.snapshot_steps
-            snaps.append({"step": cur, "R": Rn,
-                          "value": float(n) * args.snapshot_steps / (tt * 1e-3),
-                          "ms_per_step": tt / args.snapshot_steps,
-                          "pair_force_ms": fm, "in_range_ordered_pairs": pp,
-                          "roofline_frac": FLOP_PER_PAIR * pp / (fm * 1e-3) * 1e-12 / peak_tflops})
+            m = measure_point(sim, torch, flush, n, args.snapshot_steps, 10, fma_tflops)
+            m.update(step=cur, R=Rn, list=list_info(sim, use_list))
+            m["roofline_frac"] = m.pop("frac")
+            m["pair_force_ms"] = m["kernel_ms"]
+            snaps.append(m)
         out["snapshots"] = snaps
 
+    # ---- the whole shrinking schedule in one call (reading R26: up to step 17 800 for C3) ----
+    if solo and args.schedule_steps > 0:
+        ss, _, _ = make_sim(binding, w, args, device, cpc=cpc, use_list=use_list)
+        ss.step(10)
+        ss.synchronize()
+        e0.record(ss.stream)
+        ss.step(args.schedule_steps - 10)
+        e1.record(ss.stream)
+        e1.synchronize()
+        sch_ms = e0.elapsed_time(e1)
+        _, _, _, Rend, cur = ss.get_state()
+        out["schedule_mean"] = {"steps": args.schedule_steps, "ms_per_step": sch_ms / (args.schedule_steps - 10),
+                                "value": float(n) * (args.schedule_steps - 10) / (sch_ms * 1e-3), "unit": UNIT,
+                                "end_step": cur, "end_R": Rend, "status": ss.status(), "list": list_info(ss, use_list),
+                                "how": "one lv_step(S) from the initial state, device time, no flush"}
+        ss.close()
+
+    # ---- the other BASELINE configs, one short point each (default path, tuned grids) --------
+    if solo and args.other_workloads:
+        others = {}
+        for name in args.other_workloads:
+            if name == w.name:
+                continue
+            wo = workloads.make_workload(name)
+            so, cpo, ulo = make_sim(binding, wo, args, device)
+            m = measure_point(so, torch, flush, wo.n, args.other_steps, 10, fma_tflops)
+            m.update(n_particles=wo.n, cells_per_cut=list(cpo), force_path=path, list=list_info(so, ulo))
+            others[name] = m
+            so.close()
+        out["workloads"] = others
+
     # ---- oracle beside it (rank 0, N = 1 only) -----------------------------
-    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+    if solo and not args.no_cpu_baseline:
         out["cpu_baseline"] = cpu_baseline(args.workload, args.cpu_seconds)
     sim.close()
     if rank == 0:
         print(json.dumps(out))
+
+
+def config_of(w, start_step, extra=None):
+    """The same workload keys in both arms (the driver compares them)."""
+    c = {"workload": f"{w.name} (BASELINE.json configs[{int(w.name[1]) - 1}]): N={w.n}, {w.n_types} types"
+                     if w.name[0] == "C" and w.name[1:].isdigit() else w.name,
+         "n_particles": w.n, "start_step": start_step}
+    if extra:
+        c.update(extra)
+    return c
+
 
 
 # ------------------------------------------------------------ oracle timing
@@ -490,10 +600,34 @@ def cpu_baseline(name, budget_s):
     t0 = time.perf_counter()
     x, v, bad = oracle.step(p, x, v, w.type, step0=1, nsteps=m)
     dt = time.perf_counter() - t0
-    return {"value": w.n * m / dt, "unit": UNIT, "cores": oracle.max_threads(), "kind": "oracle",
-            "sample": f"{m} full-size steps (N={w.n}) of {w.name} from its initial state, "
-                      f"fp64, OpenMP over particles, {dt:.1f} s",
-            "ms_per_step": dt / m * 1e3}
+    out = {"value": w.n * m / dt, "unit": UNIT, "cores": oracle.max_threads(), "kind": "oracle",
+           "sample": f"{m} full-size steps (N={w.n}) of {w.name} from its initial state, "
+                     f"fp64, OpenMP over particles, {dt:.1f} s",
+           "ms_per_step": dt / m * 1e3}
+    # the same oracle on ONE core ("single-thread and OpenMP-all-cores"): a child
+    # process with OMP_NUM_THREADS=1 -- the thread count of an OpenMP runtime is fixed at start
+    try:
+        import subprocess
+        env = dict(os.environ, OMP_NUM_THREADS="1")
+        r = subprocess.run([sys.executable, os.path.abspath(__file__), "--oracle-single-thread", "--workload", name],
+                           env=env, capture_output=True, text=True, timeout=300)
+        out["single_thread"] = json.loads(r.stdout.strip().splitlines()[-1])
+    except Exception as e:              # a reported baseline: never fails the bench
+        out["single_thread"] = {"error": repr(e)[:200]}
+    return out
+
+
+def oracle_single_thread(name):
+    """Child of cpu_baseline (OMP_NUM_THREADS=1): two full-size oracle steps on one core."""
+    import oracle
+    w = workloads.make_workload(name)
+    p = oracle.params_from_workload(w)
+    x, v = w.pos.astype(np.float64), w.vel.astype(np.float64)
+    t0 = time.perf_counter()
+    x, v, bad = oracle.step(p, x, v, w.type, step0=0, nsteps=2)
+    dt = time.perf_counter() - t0
+    print(json.dumps({"value": w.n * 2 / dt, "unit": UNIT, "cores": oracle.max_threads(),
+                      "ms_per_step": dt / 2 * 1e3, "sample": f"2 full-size steps (N={w.n}) of {w.name}, fp64"}))
 
 
 def run_reference(args):
@@ -534,7 +668,7 @@ def run_reference(args):
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
         "data": "synthetic",
-        "config": {"workload": f"{w.name}: {sample}", "n_particles": n, "start_step": 0},
+        "config": config_of(workloads.make_workload(args.workload, state=False), 0, extra={"sample": sample, "sample_n_particles": n}),
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": oracle.max_threads(),
                          "kind": "oracle", "sample": f"{args.steps} {sample} of {w.name}, fp64"},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -553,10 +687,19 @@ def main():
     ap.add_argument("--start-step", type=int, default=0)
     ap.add_argument("--cells-per-cut", type=int, nargs="*", default=None)
     ap.add_argument("--force-kernel", type=int, default=None,
-                    help="lv_set_option(LV_OPT_FORCE_KERNEL): 0 simple, 1 queued, 2 segments (default), 3 packed f32x2")
-    ap.add_argument("--neighbour-list", type=float, nargs=2, default=None, metavar=("SKIN", "CAP"),
-                    help="lv_set_neighbour_list: time the skin-list variant instead of the per-step rebuild")
-    ap.add_argument("--no-variants", action="store_true", help="skip the skin-list variant")
+                    help="lv_set_option(LV_OPT_FORCE_KERNEL): 0 simple, 1 queued, 2 segments (default), 3 packed f32x2, "
+                         "4 tile (shared candidate stream); anything but 2 switches the neighbour list off")
+    ap.add_argument("--tile-substreams", type=int, default=None)
+    ap.add_argument("--no-list", action="store_true",
+                    help="headline without the skin neighbour list: cells rebuilt every step, cell-walk force kernel")
+    ap.add_argument("--skin", type=float, default=0.0, help="skin of the neighbour list (<= 0: automatic)")
+    ap.add_argument("--resident-steps", type=int, default=500)
+    ap.add_argument("--schedule-steps", type=int, default=-1,
+                    help="steps of the whole-schedule run (-1: 17800 for C3, else 0 = skip)")
+    ap.add_argument("--other-workloads", nargs="*", default=["C1", "C2", "C4", "C5"])
+    ap.add_argument("--other-steps", type=int, default=20)
+    ap.add_argument("--oracle-single-thread", action="store_true", help=argparse.SUPPRESS)
+    ap.add_argument("--no-variants", action="store_true", help="skip the variants and the observables")
     ap.add_argument("--small-replicas", type=int, default=16,
                     help="size of the concurrent small-droplet replica set of the variants leg (0: skip)")
     ap.add_argument("--e2e-steps", type=int, default=0)
@@ -565,10 +708,12 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     ap.add_argument("--reference-budget-s", type=float, default=150.0)
-    ap.add_argument("--force-traffic-bytes", type=float, default=None,
-                    help="dram bytes per launch of the force kernel from the committed ncu capture")
     args = ap.parse_args()
-    if args.impl == "reference":
+    if args.schedule_steps < 0:
+        args.schedule_steps = 17800 if (args.workload == "C3" and args.start_step == 0) else 0
+    if args.oracle_single_thread:
+        oracle_single_thread(args.workload)
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_lv(args)

@@ -189,7 +189,8 @@ int lv_set_option(lv_sim *s, int option, int value);
  *             first).
  *   capacity  > 0: the list pool holds capacity entries per NP ON AVERAGE (4 * capacity bytes per
  *             NP of workspace; a crowded NP may use more than its share); -1: automatic, 1024
- *             entries per NP but at most 2 GiB; 0 (default): the variant is off and every step
+ *             entries per NP but at most 2 GiB, and no list at all below 16 384 NPs (such a
+ *             step is bound by launch latency, not by the force kernel); 0 (default): the variant is off and every step
  *             rebuilds the cells, as the paper does.
  * The list is built in two passes (count the lengths, scan them, fill): every NP owns one
  * contiguous run of the pool, and 8, 16 or 32 lanes share an NP in the force kernel (chosen on

@@ -546,6 +546,11 @@ size_t lv_workspace_bytes(const lv_sim *cs)
     lv_sim *s = const_cast<lv_sim *>(cs);
     if (!s || !s->types_set || !s->sched_set) return 0;
     if (derive_grid(s) != LV_OK) return 0;
+    if (s->list_cap == -1 && s->n < 16384) {       // as lv_bind will decide
+        lv_sim t = *s;
+        t.list_cap = 0;
+        return layout_of(&t).total;
+    }
     return layout_of(s).total;
 }
 
@@ -554,6 +559,9 @@ int lv_bind(lv_sim *s, void *workspace_dev, size_t workspace_bytes, void *cuda_s
     if (!s) return LV_E_ARG;
     if (!s->types_set || !s->sched_set) return LV_E_ORDER;
     if (s->bound) return LV_E_ORDER;
+    // automatic list: a small droplet is bound by launch latency, and the list step has more
+    // (mostly idle) launches than the cell step -- keep the cells there
+    if (s->list_cap == -1 && s->n < 16384) { s->list_cap = 0; s->skin = 0.0; }
     if (s->list_cap != 0 && s->sort_mode != LV_SORT_COUNTING) return LV_E_ARG;
     int rc = derive_grid(s);
     if (rc != LV_OK) return rc;

@@ -76,7 +76,9 @@ struct LvDevState {
     unsigned int list_ok;
     unsigned int list_lanes;       // lanes that share one NP's list in the force kernel (8, 16 or 32)
     unsigned int n_fallback;       // steps taken on the cell kernel since lv_set_state
-    unsigned int pad;
+    // 1 after lv_set_state: the first step runs on the cell kernel and the list is built at the
+    // second -- a list pays only if steps follow (set_state / step(1) / get_state loops)
+    unsigned int list_defer;
     unsigned long long list_total; // entries counted by the count pass that is under way
     unsigned long long list_used;  // entries the last count needed
 };

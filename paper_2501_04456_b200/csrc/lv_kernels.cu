@@ -151,7 +151,9 @@ k_scan_cells(uint32_t n_items, uint32_t *__restrict__ cnt, uint32_t *__restrict_
 {
     if (skipped(guard)) return;
     // scan of the list lengths: a list that did not fit is counted again only every 64th step
-    if (list_guard != nullptr && list_guard->list_ok == 0u && (list_guard->step & 63) != 0) return;
+    if (list_guard != nullptr && list_guard->list_ok == 0u &&
+        ((list_guard->step & 63) != 0 || list_guard->list_defer != 0u))
+        return;
     __shared__ uint32_t s_warp[kScanThreads / 32];
     __shared__ uint32_t s_tile, s_excl;
     if (threadIdx.x == 0) s_tile = atomicAdd(scan_ticket, 1u);   // tiles start in ticket order
@@ -532,8 +534,9 @@ k_pair_force_s(const __grid_constant__ LvDev P, const float4 *__restrict__ pos,
     constexpr bool kList = kMode >= 2;          // 2: fill the list, 3: count its rows
     constexpr bool kCount = kMode == 3;
     if (kList && skipped(st)) return;
-    // a list that did not fit its pool is counted again only every 64th step
-    if (kCount && st->list_ok == 0u && (st->step & 63) != 0) return;
+    // a list that did not fit its pool is counted again only every 64th step; none is built at
+    // the first step after lv_set_state
+    if (kCount && st->list_ok == 0u && ((st->step & 63) != 0 || st->list_defer != 0u)) return;
     if (kMode == 2 && st->list_ok == 0u) return;
     // cell kernel of a list step (st given): only while the list is not in use
     if (kMode == 0 && st != nullptr && st->list_ok != 0u) return;
@@ -962,7 +965,7 @@ k_pair_force_rows(const __grid_constant__ LvDev P, const float4 *__restrict__ po
 __global__ void k_list_check(int n, uint32_t pool, LvDevState *st)
 {
     if (skipped(st)) return;
-    if (st->list_ok == 0u && (st->step & 63) != 0) return;       // not counted this step
+    if (st->list_ok == 0u && ((st->step & 63) != 0 || st->list_defer != 0u)) return;   // not counted this step
     const unsigned long long total = st->list_total;
     const bool fits = total <= (unsigned long long)pool;
     st->list_ok = fits ? 1u : 0u;
@@ -1025,6 +1028,10 @@ k_update(const __grid_constant__ LvDev P, const float4 *__restrict__ posB_,
         s_n = n0;
         s_rebuilt = kList ? st->rebuild[n0 & 1] : 1u;
         s_R = lv_radius_of(P.sched_mode, P.R0, P.R1, P.sched_steps, n0 + 1);
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {                            // off the block's critical path
+        const long long n0 = s_n;
         __threadfence();
         if (atomicAdd(&st->ticket, 1u) == gridDim.x - 1) {
             st->ticket = 0u;
@@ -1033,12 +1040,16 @@ k_update(const __grid_constant__ LvDev P, const float4 *__restrict__ posB_,
                 st->rebuild[n0 & 1] = 0u;              // ... and this step's rebuild flag
                 if (st->list_ok == 0u) {               // on the cell kernel: every step rebuilds the cells
                     st->rebuild[(n0 + 1) & 1] = 1u;
-                    st->n_fallback += 1u;
+                    if (st->list_defer != 0u) {        // first step after lv_set_state: the next one builds the list
+                        st->list_defer = 0u;
+                        st->list_ok = 1u;
+                    } else {
+                        st->n_fallback += 1u;
+                    }
                 }
             }
         }
     }
-    __syncthreads();
     const long long n = s_n;
     const bool rebuilt = s_rebuilt != 0u;
     if (i >= P.n) return;
@@ -1129,8 +1140,9 @@ k_pack_state(int n, int n_types, const float *__restrict__ pos, const float *__r
         st->rebuild[step & 1] = 1u;            // skin list: the first step builds it
         st->rebuild[(step + 1) & 1] = 0u;
         st->n_rebuilds = 0u;
-        st->list_ok = 1u;
-        st->list_lanes = 32u;
+        st->list_ok = 0u;
+        st->list_defer = 1u;
+        st->list_lanes = 8u;
         st->list_total = 0ull;
         st->list_used = 0ull;
         st->n_fallback = 0u;

@@ -15,7 +15,7 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 def test_bench_line_schema():
     cmd = [sys.executable, os.path.join(ROOT, "bench.py"), "--workload", "C2", "--steps", "20",
-           "--warmup", "3", "--no-cpu-baseline", "--no-variants", "--snapshots"]
+           "--warmup", "3", "--no-cpu-baseline", "--no-variants", "--snapshots", "--other-workloads"]
     r = subprocess.run(cmd, capture_output=True, text=True, timeout=600, cwd=ROOT)
     assert r.returncode == 0, r.stderr[-2000:]
     lines = [ln for ln in r.stdout.strip().splitlines() if ln.startswith("{")]
@@ -39,3 +39,4 @@ def test_bench_line_schema():
     assert e["h2d_bytes_per_step"] == 28 * n and e["d2h_bytes_per_step"] >= 28 * n
     assert 0.0 < e["value"] < d["value"]          # copies inside the timed region
     assert "workload" in d["config"] and "model" not in d["config"]
+    assert d["config"]["force_path"] == "list" and d["list"]["fallback_steps_in_timed_region"] == 0

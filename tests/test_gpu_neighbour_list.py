@@ -46,12 +46,18 @@ def test_first_step_forces_and_counts_against_oracle(B, orc, name, n, cpc, skin,
     p = orc.params_from_workload(w)
     Fo, So, co, _ = orc.pair_forces(p, w.pos, w.type, "cells")
     sim = B.Simulation.from_workload(w, cells_per_cut=cpc, neighbour_list=(skin, cap))
-    sim.step(1)                                   # builds the list, forces of the initial state
+    sim.step(1)                                   # first step after lv_set_state: the cell kernel
     Fg, cg = sim.get_forces()
     assert np.array_equal(cg, co)                 # neighbour counts bit-exact
     assert force_error(Fg, Fo, So) <= FORCE_TOL
+    assert sim.rebuild_count() == 0
+    x1, v1, t1, R1, st1 = sim.get_state()
+    sim.step(1)                                   # builds the list; forces of the state after step 1
     assert sim.rebuild_count() == 1
-    sim.get_state()
+    Fl, cl = sim.get_forces()
+    Fo1, So1, co1, _ = orc.pair_forces(p, x1, t1, "cells")
+    assert np.array_equal(cl, co1)
+    assert force_error(Fl, Fo1, So1) <= FORCE_TOL
     sim.close()
 
 
@@ -137,12 +143,12 @@ def test_pool_too_small_falls_back_to_the_cells(B):
     Fl, cl = lst.get_forces()
     Fc, cc = cel.get_forces()
     assert np.array_equal(cl, cc) and np.array_equal(Fl, Fc) and cc.sum() > 0
-    assert lst.status() == B.ST_LIST_OVERFLOW
     lst.step(70); cel.step(70)                    # past a re-count (every 64th step)
+    assert lst.status() == B.ST_LIST_OVERFLOW
     a, b = lst.get_state(), cel.get_state()       # no LV_E_CAPACITY any more
     assert np.array_equal(a[0], b[0]) and np.array_equal(a[1], b[1]) and a[4] == b[4] == 71
     st = lst.list_stats()
-    assert st["fallback_steps"] == 71 and st["entries_used"] > st["pool_entries"]
+    assert st["fallback_steps"] == 70 and st["entries_used"] > st["pool_entries"]
     lst.close(); cel.close()
 
 

@@ -335,6 +335,17 @@ def test_bonded_pair_outside_the_grid(B, orc, fk, sub):
         lst.step(1)
         Fl, cl = lst.get_forces()
         assert np.array_equal(cl, co)
+        # ... and through the list itself (built at the second step): the moved state against
+        # a fresh cell evaluation of it
+        xs, vs, ts, _, s1 = lst.get_state()
+        lst.step(1)
+        Fl2, cl2 = lst.get_forces()
+        cel = B.Simulation.from_workload(w, load_state=False)
+        cel.set_state(xs, vs, ts, s1)
+        cel.compute_forces()
+        Fc2, cc2 = cel.get_forces()
+        assert lst.rebuild_count() == 1 and np.array_equal(cl2, cc2) and cc2[:6].sum() >= 0
+        cel.close()
         lst.close()
 
 
