@@ -45,6 +45,31 @@ def raw_metrics(report, kernel):
     raise SystemExit(f"no launch of {kernel} in {report}")
 
 
+def sass_flops(report, kernel):
+    """FP32 flop per launch from the SASS page (predicated-on thread instructions by opcode):
+    FADD + FMUL + 2 FFMA + 2 (FADD2 + FMUL2) + 4 FFMA2 -- ncu's op_fadd/fmul/ffma counters do
+    not see the packed f32x2 forms."""
+    out = subprocess.run(["ncu", "-i", report, "--page", "source", "--csv", "-k", "regex:" + kernel],
+                         capture_output=True, text=True).stdout
+    rows = list(csv.reader(out.splitlines()))
+    k = next(i for i, r in enumerate(rows) if r and r[0] == "Address")
+    hdr = rows[k]
+    isrc, it = hdr.index("Source"), hdr.index("Predicated-On Thread Instructions Executed")
+    w = {"FADD": 1, "FMUL": 1, "FFMA": 2, "FADD2": 2, "FMUL2": 2, "FFMA2": 4}
+    ops, flops = {}, 0.0
+    for r in rows[k + 1:]:
+        if len(r) <= it or r[0] == "Address" or not r[0].startswith("0x"):
+            if r and r[0] == "Kernel Name":
+                break                       # next launch of the report
+            continue
+        tok = r[isrc].split()
+        op = (tok[1] if tok[0].startswith("@") else tok[0]).split(".")[0]
+        if op in w:
+            ops[op] = ops.get(op, 0) + int(r[it])
+            flops += w[op] * int(r[it])
+    return flops, ops
+
+
 def num(m, key, scale_units=True):
     u, v = m[key]
     x = float(v.replace(",", ""))
@@ -85,8 +110,11 @@ def main():
         "l1_data_pipe_pct": num(m, "l1tex__data_pipe_lsu_wavefronts.avg.pct_of_peak_sustained_elapsed"),
         "registers": int(num(m, "launch__registers_per_thread")),
     }
-    # executed FP32 in flop terms: (fadd + fmul + 2 ffma) per clock / (SMs x 128 lanes x 2)
-    rec["executed_fp32_frac"] = (rec["fadd"] + rec["fmul"] + 2.0 * rec["ffma"]) / cyc / (rec["n_sms"] * 128 * 2)
+    # executed FP32 in flop terms per clock / (SMs x 128 lanes x 2), opcodes from the SASS page
+    flops, ops = sass_flops(a.report, a.kernel)
+    rec["fp32_flop"] = flops
+    rec["fp32_thread_inst_by_opcode"] = ops
+    rec["executed_fp32_frac"] = flops / cyc / (rec["n_sms"] * 128 * 2)
     recs = []
     if os.path.exists(OUT):
         with open(OUT) as f:
