@@ -358,9 +358,9 @@ def run_lv(args):
     if solo and not args.no_variants and args.small_replicas > 0:
         ks = 1000
         sr = {}
-        for R_ in (1, args.small_replicas):
+        for R_, batched in ((1, False), (args.small_replicas, False), (args.small_replicas, True)):
             rs = replicas.ReplicaSet(lambda seed: workloads.make_workload("P1", seed=seed), R_,
-                                     base_seed=1234, device=device)
+                                     base_seed=1234, device=device, batched=batched, steps_per_launch=10)
             rs.step(100)
             rs.synchronize()
             torch.cuda.synchronize()
@@ -368,17 +368,17 @@ def run_lv(args):
             rs.step(ks)
             rs.synchronize()
             dt_ = time.perf_counter() - t0
-            sr[R_] = {"ms_per_step_of_all": dt_ / ks * 1e3,
-                      "value": rs.n_particles * ks / dt_, "unit": UNIT}
+            sr[("%d_one_graph" % R_) if batched else str(R_)] = {
+                "ms_per_step_of_all": dt_ / ks * 1e3, "value": rs.n_particles * ks / dt_, "unit": UNIT}
             npart = rs.workloads[0].n
             rs.close()
         variants["small_replicas"] = {
-            "what": "replicas.ReplicaSet: independent P1 droplets (Table 1 row 1 shape, N = %d each) "
-                    "stepped concurrently on one GPU, one lv_sim handle and stream per replica; "
-                    "each replica bit-identical to its solo run (test_replica_set_equals_solo_runs); "
-                    "wall clock over %d resident steps, no L2 flush" % (npart, ks),
-            "replicas": {str(k): v for k, v in sr.items()},
-            "speedup": sr[args.small_replicas]["value"] / sr[1]["value"],
+            "what": "independent P1 droplets (Table 1 row 1 shape, N = %d each) on one GPU, each replica "
+                    "bit-identical to its solo run (test_replica_set_equals_solo_runs): R handles on R streams "
+                    "driven from the host, and lv_batch = ONE CUDA graph with 10 steps of every replica as "
+                    "parallel branches; wall clock over %d resident steps, no L2 flush" % (npart, ks),
+            "replicas": sr,
+            "speedup": sr["%d_one_graph" % args.small_replicas]["value"] / sr["1"]["value"],
         }
 
     # ---- NEXT-1 rows: the paper's observables on the device (synchronous calls) -------

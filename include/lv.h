@@ -334,6 +334,20 @@ typedef struct {
 int lv_render_surface(lv_sim *s, const lv_surface_map *map, void *scratch_dev, uint32_t *rgba,
                       int on_device);
 
+/* Batched replicas (the paper's use as a quick hypothesis tester at
+ * 10^4 NPs): n_sims independent handles -- each bound to its OWN stream
+ * and workspace, state loaded -- are stepped by ONE CUDA-graph launch that holds
+ * steps_per_launch (1..256) steps of every replica as parallel branches.  Replicas do not
+ * interact: each one's result is bit-identical to stepping it alone.  lv_batch_step(b, n)
+ * enqueues n steps of all replicas on the first replica's stream (the other streams are made to
+ * wait for it) and returns without synchronising; the handles stay usable for every lv_get_* /
+ * lv_set_state call.  Do not call lv_step on a member while batched steps are in flight on
+ * another stream.  The batch borrows the handles: destroy it before them. */
+typedef struct lv_batch lv_batch;
+int lv_batch_create(lv_batch **out, lv_sim **sims, int n_sims, int steps_per_launch);
+int lv_batch_step(lv_batch *b, int n);
+int lv_batch_destroy(lv_batch *b);
+
 /* Status bits LV_ST_* (host uint32, written).  Synchronises. */
 int lv_get_status(lv_sim *s, uint32_t *status);
 

@@ -35,7 +35,7 @@ SYMBOLS = ["lv_langevin_coeffs", "lv_create", "lv_set_types", "lv_set_forces",
            "lv_get_status", "lv_get_debug", "lv_launches_per_step", "lv_step_profiled",
            "lv_stage_timing", "lv_read_stage_timing",
            "lv_measure_fp32_peak", "lv_destroy", "lv_strerror",
-           "lv_last_cuda_error", "lv_version"]
+           "lv_last_cuda_error", "lv_version", "lv_batch_create", "lv_batch_step", "lv_batch_destroy"]
 
 
 class LvView(C.Structure):
@@ -118,6 +118,9 @@ def load():
     L.lv_last_cuda_error.argtypes = [vp]
     L.lv_last_cuda_error.restype = C.c_char_p
     L.lv_version.restype = C.c_char_p
+    L.lv_batch_create.argtypes = [C.POINTER(vp), C.POINTER(vp), C.c_int, C.c_int]
+    L.lv_batch_step.argtypes = [vp, C.c_int]
+    L.lv_batch_destroy.argtypes = [vp]
     _lib = L
     return L
 
@@ -132,6 +135,35 @@ def langevin_coeffs(gamma, kT, mass, dt):
 
 def _dptr(a):
     return None if a is None else a.ctypes.data_as(C.POINTER(C.c_double))
+
+
+class Batch:
+    """lv_batch: bound Simulations (own streams) stepped together by one CUDA-graph launch."""
+
+    def __init__(self, sims, steps_per_launch: int = 8):
+        self.L = load()
+        self.sims = list(sims)
+        arr = (C.c_void_p * len(self.sims))(*[s.h for s in self.sims])
+        self.h = C.c_void_p()
+        rc = self.L.lv_batch_create(C.byref(self.h), arr, len(self.sims), int(steps_per_launch))
+        if rc != 0:
+            raise LvError(rc, "lv_batch_create", self.L.lv_strerror(rc).decode())
+
+    def step(self, n: int = 1):
+        rc = self.L.lv_batch_step(self.h, int(n))
+        if rc != 0:
+            raise LvError(rc, "lv_batch_step", self.L.lv_strerror(rc).decode())
+
+    def close(self):
+        if getattr(self, "h", None):
+            self.L.lv_batch_destroy(self.h)
+            self.h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
 
 
 class Simulation:

@@ -1125,3 +1125,126 @@ const char *lv_last_cuda_error(const lv_sim *s) { return s ? s->cuda_err : ""; }
 const char *lv_version(void) { return "lv 0.1.0 (sm_100a)"; }
 
 }  // extern "C"
+
+// ---- batched replicas: R independent lv_sim handles stepped by ONE
+// CUDA-graph launch.  The graph holds one step (or `chunk` steps) of every replica as parallel
+// branches forked from and joined into the first replica's stream, so the small kernels of
+// many small droplets share the GPU without R launch sequences issued from the host.
+struct lv_batch {
+    int n = 0, chunk = 1;
+    lv_sim **sims = nullptr;
+    cudaEvent_t *ev = nullptr;          // [n]: join events; ev[0] = fork
+    cudaGraph_t graph1 = nullptr, graphk = nullptr;
+    cudaGraphExec_t exec1 = nullptr, execk = nullptr;
+};
+
+namespace {
+// capture `steps` steady-state steps of every replica into one graph
+int capture_batch(lv_batch *b, int steps, cudaGraph_t *g, cudaGraphExec_t *x)
+{
+    lv_sim *s0 = b->sims[0];
+    LV_CUDA(s0, cudaStreamBeginCapture(s0->stream, cudaStreamCaptureModeRelaxed));
+    int rc = LV_OK;
+    cudaError_t e = cudaEventRecord(b->ev[0], s0->stream);
+    for (int r = 1; r < b->n && e == cudaSuccess; ++r) e = cudaStreamWaitEvent(b->sims[r]->stream, b->ev[0], 0);
+    for (int r = 0; r < b->n && e == cudaSuccess && rc == LV_OK; ++r) {
+        lv_sim *s = b->sims[r];
+        for (int k = 0; k < steps && rc == LV_OK; ++k) {
+            s->hashed = s->sort_mode == LV_SORT_COUNTING && s->list_cap == 0;     // steady-state step
+            rc = enqueue_step(s);
+        }
+        s->hashed = false;
+        if (r > 0 && rc == LV_OK) {
+            e = cudaEventRecord(b->ev[r], s->stream);
+            if (e == cudaSuccess) e = cudaStreamWaitEvent(s0->stream, b->ev[r], 0);
+        }
+    }
+    cudaGraph_t gg = nullptr;
+    cudaError_t e2 = cudaStreamEndCapture(s0->stream, &gg);
+    if (rc == LV_OK && e != cudaSuccess) rc = cuda_fail(s0, e, "lv_batch capture");
+    if (rc == LV_OK && e2 != cudaSuccess) rc = cuda_fail(s0, e2, "cudaStreamEndCapture");
+    if (rc == LV_OK) {
+        e2 = cudaGraphInstantiate(x, gg, 0);
+        if (e2 != cudaSuccess) rc = cuda_fail(s0, e2, "cudaGraphInstantiate");
+    }
+    if (rc != LV_OK) { if (gg) cudaGraphDestroy(gg); return rc; }
+    *g = gg;
+    return LV_OK;
+}
+}  // namespace
+
+extern "C" {
+
+int lv_batch_destroy(lv_batch *b)
+{
+    if (!b) return LV_OK;
+    if (b->sims && b->n > 0 && b->sims[0]) cudaStreamSynchronize(b->sims[0]->stream);
+    if (b->exec1) cudaGraphExecDestroy(b->exec1);
+    if (b->execk) cudaGraphExecDestroy(b->execk);
+    if (b->graph1) cudaGraphDestroy(b->graph1);
+    if (b->graphk) cudaGraphDestroy(b->graphk);
+    if (b->ev) {
+        for (int r = 0; r < b->n; ++r) if (b->ev[r]) cudaEventDestroy(b->ev[r]);
+        free(b->ev);
+    }
+    free(b->sims);
+    delete b;
+    return LV_OK;
+}
+
+int lv_batch_create(lv_batch **out, lv_sim **sims, int n_sims, int steps_per_launch)
+{
+    if (!out || !sims || n_sims < 1 || n_sims > 4096 || steps_per_launch < 1 || steps_per_launch > 256) return LV_E_ARG;
+    for (int r = 0; r < n_sims; ++r) {
+        if (!sims[r]) return LV_E_ARG;
+        if (!sims[r]->bound || !sims[r]->state_set) return LV_E_ORDER;
+        if (sims[r]->stream == nullptr || sims[r]->n == 0 || sims[r]->tim_cap > 0) return LV_E_ARG;
+        for (int q = 0; q < r; ++q) if (sims[q] == sims[r]) return LV_E_ARG;
+    }
+    lv_batch *b = new (std::nothrow) lv_batch();
+    if (!b) return LV_E_NOMEM;
+    b->n = n_sims;
+    b->chunk = steps_per_launch;
+    b->sims = (lv_sim **)malloc(sizeof(lv_sim *) * n_sims);
+    b->ev = (cudaEvent_t *)calloc(n_sims, sizeof(cudaEvent_t));
+    if (!b->sims || !b->ev) { lv_batch_destroy(b); return LV_E_NOMEM; }
+    memcpy(b->sims, sims, sizeof(lv_sim *) * n_sims);
+    for (int r = 0; r < n_sims; ++r)
+        if (cudaEventCreateWithFlags(&b->ev[r], cudaEventDisableTiming) != cudaSuccess) { lv_batch_destroy(b); return LV_E_CUDA; }
+    int rc = capture_batch(b, 1, &b->graph1, &b->exec1);
+    if (rc == LV_OK && b->chunk > 1) rc = capture_batch(b, b->chunk, &b->graphk, &b->execk);
+    if (rc != LV_OK) { lv_batch_destroy(b); return rc; }
+    *out = b;
+    return LV_OK;
+}
+
+int lv_batch_step(lv_batch *b, int n)
+{
+    if (!b || n < 0) return LV_E_ARG;
+    if (n == 0) return LV_OK;
+    lv_sim *s0 = b->sims[0];
+    // everything enqueued on the replicas' own streams so far comes first
+    for (int r = 1; r < b->n; ++r) {
+        LV_CUDA(s0, cudaEventRecord(b->ev[r], b->sims[r]->stream));
+        LV_CUDA(s0, cudaStreamWaitEvent(s0->stream, b->ev[r], 0));
+    }
+    for (int r = 0; r < b->n; ++r) {
+        lv_sim *s = b->sims[r];
+        if (s->sort_mode == LV_SORT_COUNTING && s->list_cap == 0 && !s->hashed) {
+            LV_CUDA(s0, lvk_hash_count(s->dev, s->bufs, false, s0->stream));     // the graph is the steady-state step
+            s->hashed = true;
+        }
+        s->force_order_b = false;
+    }
+    int left = n;
+    while (left > 0) {
+        if (b->execk && left >= b->chunk) { LV_CUDA(s0, cudaGraphLaunch(b->execk, s0->stream)); left -= b->chunk; }
+        else { LV_CUDA(s0, cudaGraphLaunch(b->exec1, s0->stream)); left -= 1; }
+    }
+    // ... and the replicas' own streams see the result
+    LV_CUDA(s0, cudaEventRecord(b->ev[0], s0->stream));
+    for (int r = 1; r < b->n; ++r) LV_CUDA(s0, cudaStreamWaitEvent(b->sims[r]->stream, b->ev[0], 0));
+    return LV_OK;
+}
+
+}  // extern "C"

@@ -66,12 +66,16 @@ class ReplicaSet:
     hypothesis testing).  `step(n)` enqueues the n graph
     replays of every replica in slices, round robin, so that every stream
     always has work queued and the kernels of different replicas overlap on
-    the SMs.  There is no coupling between replicas: replica r of the set
-    is bit-identical to the same workload stepped alone
+    the SMs.  With `batched=True` (default) the set is an `lv_batch` instead:
+    ONE CUDA graph holds `steps_per_launch` steps of every replica as parallel
+    branches, so a step of all R droplets is one launch, not 5 R.  There is no
+    coupling between replicas: replica r of the set is bit-identical to the same
+    workload stepped alone
     (tests/test_gpu_parity.py::test_replica_set_equals_solo_runs)."""
 
     def __init__(self, make_workload, n_replicas: int, base_seed: int, device: str = "cuda:0",
-                 cells_per_cut=None, options=None, neighbour_list=None, slice_steps: int = 50):
+                 cells_per_cut=None, options=None, neighbour_list=None, slice_steps: int = 50,
+                 batched: bool = True, steps_per_launch: int = 8):
         _check_cuda_extension()
         from . import binding
         if n_replicas < 1:
@@ -81,6 +85,7 @@ class ReplicaSet:
         self.sims = [binding.Simulation.from_workload(
             w, cells_per_cut=cells_per_cut if cells_per_cut is not None else w.tuned_cells_per_cut,
             device=device, options=options, neighbour_list=neighbour_list) for w in self.workloads]
+        self.batch = binding.Batch(self.sims, steps_per_launch) if batched else None
 
     def __len__(self) -> int:
         return len(self.sims)
@@ -90,6 +95,9 @@ class ReplicaSet:
         return sum(w.n for w in self.workloads)
 
     def step(self, n: int = 1) -> None:
+        if self.batch is not None:
+            self.batch.step(n)
+            return
         done = 0
         while done < n:
             k = min(self.slice_steps, n - done)
@@ -105,6 +113,9 @@ class ReplicaSet:
         return self.sims[r].get_state(**kw)
 
     def close(self) -> None:
+        if getattr(self, "batch", None) is not None:
+            self.batch.close()
+            self.batch = None
         for s in self.sims:
             s.close()
         self.sims = []

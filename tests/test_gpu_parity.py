@@ -498,15 +498,18 @@ def test_split_invariance_and_roundtrip(B):
         s.close()
 
 
-def test_replica_set_equals_solo_runs(B, orc):
-    """NEXT-3 batched replicas: R small droplets stepped concurrently on R streams of one GPU
-    are each bit-identical to the same workload stepped alone (no coupling between
-    replicas), differ from one another (distinct seeds), and replica 0 still tracks the oracle."""
+@pytest.mark.parametrize("batched", [True, False])
+def test_replica_set_equals_solo_runs(B, orc, batched):
+    """NEXT-3 batched replicas: R small droplets stepped together -- by ONE CUDA-graph launch
+    per chunk of steps (lv_batch, parallel branches), or concurrently on R streams -- are each
+    bit-identical to the same workload stepped alone (no coupling between replicas), differ from
+    one another (distinct seeds), and replica 0 still tracks the oracle."""
     from paper_2501_04456_b200 import replicas
     mk = lambda seed: W.make_workload("C1", 1024, seed=seed)
-    rs = replicas.ReplicaSet(mk, 5, base_seed=77, slice_steps=7)
+    rs = replicas.ReplicaSet(mk, 5, base_seed=77, slice_steps=7, batched=batched, steps_per_launch=6)
     assert len(rs) == 5 and rs.n_particles == 5 * 1024
-    rs.step(40)
+    rs.step(13)                      # two chunks of 6 and a single step
+    rs.step(27)
     rs.synchronize()
     got = [rs.get_state(r) for r in range(5)]
     for r in range(5):
