@@ -205,10 +205,10 @@ int lv_set_neighbour_list(lv_sim *s, double skin, int capacity);
  * with the neighbour list on.  Synchronises. */
 int lv_get_rebuild_count(lv_sim *s, int64_t *rebuilds);
 
-/* out4 (host int64[4], written): rebuilds since lv_set_state, list entries (lengths padded to
- * a multiple of 4) the last count needed, steps taken on the cell kernel because the list did not fit, pool size
+/* out6 (host int64[6], written): rebuilds since lv_set_state, list entries the last build
+ * reserved, steps taken on the cell kernel because the list did not fit, pool size
  * in entries.  Synchronises. */
-int lv_get_list_stats(lv_sim *s, int64_t *out4);
+int lv_get_list_stats(lv_sim *s, int64_t *out6);
 
 /* Bytes of device workspace lv_bind needs (0 if types are not set). */
 size_t lv_workspace_bytes(const lv_sim *s);

@@ -227,9 +227,10 @@ class Simulation:
         return int(r.value)
 
     def list_stats(self) -> dict:
-        o = (C.c_int64 * 4)()
+        o = (C.c_int64 * 6)()
         self._check(self.L.lv_get_list_stats(self.h, o), "lv_get_list_stats")
-        return dict(rebuilds=int(o[0]), entries_used=int(o[1]), fallback_steps=int(o[2]), pool_entries=int(o[3]))
+        return dict(rebuilds=int(o[0]), entries_used=int(o[1]), fallback_steps=int(o[2]), pool_entries=int(o[3]),
+                    exact_rebuilds=int(o[4]), lanes_per_np=int(o[5]))
 
     def workspace_bytes(self) -> int:
         return int(self.L.lv_workspace_bytes(self.h))

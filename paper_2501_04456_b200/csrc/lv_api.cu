@@ -116,7 +116,7 @@ int derive_grid(lv_sim *s)
 struct Layout {
     size_t posA, velA, posB, velB, force, key_in, key_out, val_in, val_out, cell_off, sort_temp,
         sort_temp_bytes, st, staging, cell_cnt, scan_tile, scan_ticket, posP, list, list_cnt,
-        list_start, list_scan_tile, list_scan_ticket, pos_ref, total;
+        list_start, list_len, list_scan_tile, list_scan_ticket, pos_ref, total;
 };
 
 // Pool of the skin list in entries: list_cap per NP on average (a crowded NP may use more than
@@ -157,6 +157,7 @@ Layout layout_of(const lv_sim *s)
     L.list = take(4 * list_pool_of(s));
     L.list_cnt = take(s->list_cap != 0 ? 4 * (n + 1) : 0);
     L.list_start = take(s->list_cap != 0 ? 4 * (n + 1) : 0);
+    L.list_len = take(s->list_cap != 0 ? 4 * (n + 1) : 0);
     L.list_scan_tile = take(s->list_cap != 0 ? 8 * ((n + 1 + kScanTile - 1) / kScanTile) : 0);
     L.list_scan_ticket = take(4);
     L.pos_ref = take(s->list_cap != 0 ? 16 * n : 0);
@@ -334,29 +335,102 @@ void free_timing(lv_sim *s)
 
 // Capture one step into a graph (nothing executes during capture).  The graph
 // is static: the step index and the radius live in device memory.
+// List step as a graph with an IF node: [condition kernel] -> IF(rebuild flag){ rebuild chain:
+// stages 0..2 } -> list force, cell force (guarded) -> update.  The body is captured on a
+// helper stream into the conditional node's body graph.
+int capture_list_step(lv_sim *s, cudaGraph_t g, cudaGraph_t *body_out)
+{
+    cudaGraphConditionalHandle h;
+    LV_CUDA(s, cudaGraphConditionalHandleCreate(&h, g, 0, 0));
+    LV_CUDA(s, cudaStreamBeginCaptureToGraph(s->stream, g, nullptr, nullptr, 0, cudaStreamCaptureModeRelaxed));
+    int rc = LV_OK;
+    cudaError_t e = lvk_list_cond((unsigned long long)h, s->bufs, s->stream);
+    cudaStream_t helper = nullptr;
+    if (e == cudaSuccess) {
+        cudaStreamCaptureStatus cst;
+        const cudaGraphNode_t *deps = nullptr;
+        size_t nd = 0;
+        cudaGraph_t cg = nullptr;
+        e = cudaStreamGetCaptureInfo_v2(s->stream, &cst, nullptr, &cg, &deps, &nd);
+        cudaGraphNodeParams np = {};
+        np.type = cudaGraphNodeTypeConditional;
+        np.conditional.handle = h;
+        np.conditional.type = cudaGraphCondTypeIf;
+        np.conditional.size = 1;
+        cudaGraphNode_t cn = nullptr;
+        if (e == cudaSuccess) e = cudaGraphAddNode(&cn, cg, deps, nd, &np);
+        if (e == cudaSuccess) e = cudaStreamUpdateCaptureDependencies(s->stream, &cn, 1, cudaStreamSetCaptureDependencies);
+        if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&helper, cudaStreamNonBlocking);
+        if (e == cudaSuccess) {
+            cudaGraph_t body = np.conditional.phGraph_out[0];
+            *body_out = body;
+            e = cudaStreamBeginCaptureToGraph(helper, body, nullptr, nullptr, 0, cudaStreamCaptureModeRelaxed);
+            if (e == cudaSuccess) {
+                cudaStream_t keep = s->stream;
+                s->stream = helper;                 // the stage functions launch on s->stream
+                for (int k = 0; k < 3 && rc == LV_OK; ++k) rc = enqueue_stage(s, k, true);
+                s->stream = keep;
+                cudaGraph_t tmp = nullptr;
+                cudaError_t e2 = cudaStreamEndCapture(helper, &tmp);
+                if (e == cudaSuccess) e = e2;
+            }
+        }
+    }
+    for (int k = 3; k < LV_N_STAGES && rc == LV_OK && e == cudaSuccess; ++k) rc = enqueue_stage(s, k, true);
+    cudaGraph_t gout = nullptr;
+    cudaError_t e3 = cudaStreamEndCapture(s->stream, &gout);
+    if (helper) cudaStreamDestroy(helper);
+
+    if (rc != LV_OK) return rc;
+    if (e != cudaSuccess) return cuda_fail(s, e, "capture of the list step");
+    if (e3 != cudaSuccess) return cuda_fail(s, e3, "cudaStreamEndCapture");
+    return LV_OK;
+}
+
+// Capture one step into a graph (nothing executes during capture).  The graph
+// is static: the step index and the radius live in device memory.
 int build_graph(lv_sim *s)
 {
     if (s->stream == nullptr || s->n == 0) return LV_OK;   // legacy stream: direct launches
-    LV_CUDA(s, cudaStreamBeginCapture(s->stream, cudaStreamCaptureModeRelaxed));
-    s->hashed = s->sort_mode == LV_SORT_COUNTING && s->list_cap == 0;   // the graph is the steady-state step
-    int rc = enqueue_step(s);
-    s->hashed = false;
-    cudaGraph_t g = nullptr;
-    cudaError_t e = cudaStreamEndCapture(s->stream, &g);
-    if (rc != LV_OK) { if (g) cudaGraphDestroy(g); return rc; }     // the capture has been ended above
-    if (e != cudaSuccess) return cuda_fail(s, e, "cudaStreamEndCapture");
-    s->graph = g;
-    size_t nn = 0;
-    LV_CUDA(s, cudaGraphGetNodes(g, nullptr, &nn));
-    cudaGraphNode_t *nodes = (cudaGraphNode_t *)malloc(sizeof(cudaGraphNode_t) * (nn ? nn : 1));
-    if (!nodes) { cudaGraphDestroy(g); s->graph = nullptr; return LV_E_NOMEM; }
-    cudaError_t e2 = cudaGraphGetNodes(g, nodes, &nn);
-    int kernels = 0;
-    for (size_t i = 0; e2 == cudaSuccess && i < nn; ++i) {
-        cudaGraphNodeType t;
-        if (cudaGraphNodeGetType(nodes[i], &t) == cudaSuccess && t == cudaGraphNodeTypeKernel) ++kernels;
+    cudaGraph_t g = nullptr, body = nullptr;
+    int rc = LV_OK;
+    if (s->list_cap != 0) {
+        LV_CUDA(s, cudaGraphCreate(&g, 0));
+        rc = capture_list_step(s, g, &body);
+        if (rc != LV_OK) { cudaGraphDestroy(g); return rc; }
+    } else {
+        LV_CUDA(s, cudaStreamBeginCapture(s->stream, cudaStreamCaptureModeRelaxed));
+        s->hashed = s->sort_mode == LV_SORT_COUNTING;      // the graph is the steady-state step
+        rc = enqueue_step(s);
+        s->hashed = false;
+        cudaError_t e = cudaStreamEndCapture(s->stream, &g);
+        if (rc != LV_OK) { if (g) cudaGraphDestroy(g); return rc; }     // the capture has been ended above
+        if (e != cudaSuccess) return cuda_fail(s, e, "cudaStreamEndCapture");
     }
-    free(nodes);
+    s->graph = g;
+    // kernels of one step (the IF node's body included)
+    int kernels = 0;
+    cudaError_t e2 = cudaSuccess;
+    {
+        cudaGraph_t todo[2] = {g, body};
+        for (int q = 0; q < 2 && todo[q] && e2 == cudaSuccess; ++q) {
+            size_t nn = 0;
+            e2 = cudaGraphGetNodes(todo[q], nullptr, &nn);
+            cudaGraphNode_t *nodes = (cudaGraphNode_t *)malloc(sizeof(cudaGraphNode_t) * (nn ? nn : 1));
+            if (!nodes) { cudaGraphDestroy(g); s->graph = nullptr; return LV_E_NOMEM; }
+            if (e2 == cudaSuccess) e2 = cudaGraphGetNodes(todo[q], nodes, &nn);
+            for (size_t i = 0; e2 == cudaSuccess && i < nn; ++i) {
+                cudaGraphNodeType t;
+                if (cudaGraphNodeGetType(nodes[i], &t) != cudaSuccess) {
+                    (void)cudaGetLastError();       // the conditional node: not a kernel; leave no stale error behind
+                    continue;
+                }
+                if (t == cudaGraphNodeTypeKernel) ++kernels;
+            }
+            free(nodes);
+        }
+    }
+    (void)cudaGetLastError();
     if (e2 == cudaSuccess) e2 = cudaGraphInstantiate(&s->graph_exec, g, 0);
     if (e2 != cudaSuccess) {          // leave no half-built graph behind
         cudaGraphDestroy(g);
@@ -516,9 +590,10 @@ int lv_set_neighbour_list(lv_sim *s, double skin, int capacity)
     return LV_OK;
 }
 
-int lv_get_list_stats(lv_sim *s, int64_t *out4)
+int lv_get_list_stats(lv_sim *s, int64_t *out6)
 {
-    if (!s || !out4) return LV_E_ARG;
+    int64_t *out4 = out6;
+    if (!s || !out6) return LV_E_ARG;
     if (!s->bound) return LV_E_ORDER;
     LvDevState h;
     LV_CUDA(s, cudaMemcpyAsync(&h, s->bufs.st, sizeof(h), cudaMemcpyDeviceToHost, s->stream));
@@ -527,6 +602,8 @@ int lv_get_list_stats(lv_sim *s, int64_t *out4)
     out4[1] = (int64_t)h.list_used;
     out4[2] = (int64_t)h.n_fallback;
     out4[3] = (int64_t)s->dev.list_pool;
+    out6[4] = (int64_t)h.n_exact;
+    out6[5] = (int64_t)h.list_lanes;
     return LV_OK;
 }
 
@@ -587,6 +664,7 @@ int lv_bind(lv_sim *s, void *workspace_dev, size_t workspace_bytes, void *cuda_s
     B.list = (uint32_t *)(w + L.list);
     B.list_cnt = (uint32_t *)(w + L.list_cnt);
     B.list_start = (uint32_t *)(w + L.list_start);
+    B.list_len = (uint32_t *)(w + L.list_len);
     B.list_scan_tile = (unsigned long long *)(w + L.list_scan_tile);
     B.list_scan_ticket = (unsigned int *)(w + L.list_scan_ticket);
     B.pos_ref = (float4 *)(w + L.pos_ref);

@@ -80,7 +80,15 @@ struct LvDevState {
     // second -- a list pays only if steps follow (set_state / step(1) / get_state loops)
     unsigned int list_defer;
     unsigned long long list_total; // entries counted by the count pass that is under way
-    unsigned long long list_used;  // entries the last count needed
+    unsigned long long list_used;  // entries the last build reserved
+    // 1: list_len[] holds the lengths of a valid list in the present slot order, so the next
+    // rebuild can size the new lists from them and fill in ONE walk
+    unsigned int list_prev;
+    // raised during a rebuild when the one-walk build cannot be used or a list outgrew its
+    // reserve: the exact two-pass build (count, scan, fill) of the same step takes over
+    unsigned int list_redo;
+    unsigned int n_exact;          // rebuilds done by the exact two-pass build since lv_set_state
+    unsigned int pad;
 };
 
 struct LvBufs {
@@ -108,8 +116,9 @@ struct LvBufs {
     // list_cnt = padded lengths (input of the scan, zero between builds), list_start = their
     // exclusive scan; pos_ref = positions at the last build.
     uint32_t *list;
-    uint32_t *list_cnt;      // [n + 1]
+    uint32_t *list_cnt;      // [n + 1] reserved lengths (input of the scan, zero between builds)
     uint32_t *list_start;    // [n + 1]
+    uint32_t *list_len;      // [n] true lengths, padded to a multiple of 4
     unsigned long long *list_scan_tile;
     unsigned int *list_scan_ticket;
     float4 *pos_ref;
@@ -143,6 +152,8 @@ cudaError_t lvk_rank_gather(const LvDev &P, const LvBufs &B, bool packed, bool g
 // skin list: build from the cell structures (guarded), force from the list, update in list order
 // count (rows per warp) -> scan (tile offsets, pool check) -> fill, all guarded
 cudaError_t lvk_list_build(const LvDev &P, const LvBufs &B, cudaStream_t st);
+// sets the condition of the graph's IF node (the rebuild chain) from this step's rebuild flag
+cudaError_t lvk_list_cond(unsigned long long handle, const LvBufs &B, cudaStream_t st);
 // cell kernel of a list step: runs only while the list does not fit its pool
 cudaError_t lvk_pair_force_fallback(const LvDev &P, const LvBufs &B, cudaStream_t st);
 cudaError_t lvk_pair_force_list(const LvDev &P, const LvBufs &B, cudaStream_t st);

@@ -147,13 +147,15 @@ constexpr int kScanThreads = kScanTile / kScanItems;
 __global__ void __launch_bounds__(kScanThreads)
 k_scan_cells(uint32_t n_items, uint32_t *__restrict__ cnt, uint32_t *__restrict__ off,
              volatile unsigned long long *scan_tile, unsigned int *scan_ticket,
-             const LvDevState *guard, const LvDevState *list_guard)
+             const LvDevState *guard, const LvDevState *list_guard, int list_mode)
 {
     if (skipped(guard)) return;
-    // scan of the list lengths: a list that did not fit is counted again only every 64th step
-    if (list_guard != nullptr && list_guard->list_ok == 0u &&
-        ((list_guard->step & 63) != 0 || list_guard->list_defer != 0u))
-        return;
+    // scan of the list lengths (list_mode 1: one-walk build, 2: exact build): only for the build
+    // that is on; a list that did not fit is counted again only every 64th step
+    if (list_guard != nullptr) {
+        if ((list_mode == 1) != (list_guard->list_redo == 0u)) return;
+        if (list_guard->list_ok == 0u && ((list_guard->step & 63) != 0 || list_guard->list_defer != 0u)) return;
+    }
     __shared__ uint32_t s_warp[kScanThreads / 32];
     __shared__ uint32_t s_tile, s_excl;
     if (threadIdx.x == 0) s_tile = atomicAdd(scan_ticket, 1u);   // tiles start in ticket order
@@ -518,6 +520,15 @@ constexpr int kSegCap = LV_S_SEGCAP;       // segments per lane between walks
 constexpr int kSChunk = LV_S_CHUNK;
 
 
+struct LvListArgs {          // list modes of k_pair_force_s
+    uint32_t *list;
+    uint32_t *cnt;                   // reserved lengths (count mode writes them)
+    const uint32_t *start;           // exclusive scan of the reserved lengths (fill modes)
+    uint32_t *len;                   // true padded lengths (fill modes write them)
+    unsigned long long *scan_tile;   // look-back words of the scan over the lengths (re-armed by count)
+    unsigned int *scan_ticket;
+};
+
 // kMode 0: forces, scalar walk.  1: forces, packed walk.  2: no forces -- the same row and
 // walk phases with the cut-off widened by the skin EMIT the in-range slots into the lane's
 // column of its warp's tile of the skin neighbour list (lv_set_neighbour_list).
@@ -525,15 +536,18 @@ template <bool kCharged, int kMode>
 __global__ void __launch_bounds__(kSThreads, LV_S_MINBLOCKS)
 k_pair_force_s(const __grid_constant__ LvDev P, const float4 *__restrict__ pos,
                const uint32_t *__restrict__ off, float4 *__restrict__ force,
-               const float *__restrict__ posP, uint32_t *__restrict__ list,
-               uint32_t *__restrict__ list_cnt, const uint32_t *__restrict__ list_start,
-               unsigned long long *__restrict__ list_scan_tile, unsigned int *__restrict__ list_scan_ticket,
-               LvDevState *st)
+               const float *__restrict__ posP, const LvListArgs LA, LvDevState *st)
 {
     constexpr bool kPacked = kMode == 1;
-    constexpr bool kList = kMode >= 2;          // 2: fill the list, 3: count its rows
+    // 2: fill the lists (exact build), 3: count their lengths (exact build), 4: fill in one walk
+    // into runs reserved from the previous lengths
+    constexpr bool kList = kMode >= 2;
     constexpr bool kCount = kMode == 3;
+    constexpr bool kFill = kMode == 2 || kMode == 4;
+    constexpr bool kOpt = kMode == 4;
     if (kList && skipped(st)) return;
+    if (kOpt && st->list_redo != 0u) return;               // the one-walk build is off for this rebuild
+    if ((kCount || kMode == 2) && st->list_redo == 0u) return;      // ... or it has done the job
     // a list that did not fit its pool is counted again only every 64th step; none is built at
     // the first step after lv_set_state
     if (kCount && st->list_ok == 0u && ((st->step & 63) != 0 || st->list_defer != 0u)) return;
@@ -554,12 +568,18 @@ k_pair_force_s(const __grid_constant__ LvDev P, const float4 *__restrict__ pos,
     const uint32_t self = live ? (uint32_t)i : 0u;
     // list mode: the lane's column of its warp's tile, and whether it overflowed
     if (kCount) {                       // re-arm the scan of the list lengths that follows
-        if (gtid < (int)P.n_list_tiles) list_scan_tile[gtid] = 0ull;
-        if (gtid == 0) { *list_scan_ticket = 0u; list_cnt[P.n] = 0u; }
+        if (gtid < (int)P.n_list_tiles) LA.scan_tile[gtid] = 0ull;
+        if (gtid == 0) { *LA.scan_ticket = 0u; LA.cnt[P.n] = 0u; }
     }
-    // fill mode: the NP's own list (list_start = exclusive scan of the padded lengths), written
-    // four entries (16 bytes) at a time
-    uint4 *col = kMode == 2 && gtid < P.n ? reinterpret_cast<uint4 *>(list + list_start[P.n - 1 - gtid]) : nullptr;
+    // fill modes: the NP's own list (start = exclusive scan of the reserved lengths), written
+    // four entries (16 bytes) at a time; cap = its reserve (exact build: its counted length)
+    uint4 *col = nullptr;
+    int cap = 0;
+    if (kFill && gtid < P.n) {
+        const uint32_t b0 = LA.start[P.n - 1 - gtid];
+        col = reinterpret_cast<uint4 *>(LA.list + b0);
+        cap = (int)(LA.start[P.n - gtid] - b0);
+    }
     uint4 ebuf = make_uint4(0u, 0u, 0u, 0u);
     const float4 pi = pos[self];
     const int a = live ? __float_as_int(pi.w) : 0;
@@ -610,7 +630,7 @@ k_pair_force_s(const __grid_constant__ LvDev P, const float4 *__restrict__ pos,
                             ebuf.y = q == 1 ? jj[u] : ebuf.y;
                             ebuf.z = q == 2 ? jj[u] : ebuf.z;
                             ebuf.w = jj[u];
-                            if (q == 3) col[cnt >> 2] = ebuf;
+                            if (q == 3 && cnt < cap) col[cnt >> 2] = ebuf;     // cap is a multiple of 4
                         }
                         ++cnt;
                     }
@@ -832,18 +852,20 @@ k_pair_force_s(const __grid_constant__ LvDev P, const float4 *__restrict__ pos,
         // holds the NP's own slot, which the force kernel rejects by j != i
         if (kCount) {
             const uint32_t padded = live ? ((uint32_t)cnt + 3u) & ~3u : 0u;
-            if (live) list_cnt[i] = padded;
+            if (live) LA.cnt[i] = padded;
             const uint32_t wsum = __reduce_add_sync(kFull, padded);
             if ((gtid & 31) == 0 && wsum) atomicAdd(&st->list_total, (unsigned long long)wsum);
         } else {
             const int q = cnt & 3;              // the last, partial group: padded with the NP's own slot
-            if (live && q != 0) {
+            if (live && q != 0 && cnt < cap) {
                 ebuf.y = q > 1 ? ebuf.y : self;
                 ebuf.z = q > 2 ? ebuf.z : self;
                 ebuf.w = self;
                 col[cnt >> 2] = ebuf;
             }
-            if (gtid == 0) st->n_rebuilds += 1u;
+            if (live) LA.len[i] = ((uint32_t)cnt + 3u) & ~3u;
+            // one-walk build: a list that outgrew its reserve hands the rebuild to the exact build
+            if (kOpt && live && cnt > cap) st->list_redo = 1u;
         }
         return;
     }
@@ -866,6 +888,7 @@ template <bool kCharged, int S>
 __device__ __forceinline__ void rows_body(const LvDev &P, const float4 *__restrict__ pos,
                                           const uint32_t *__restrict__ list,
                                           const uint32_t *__restrict__ list_start,
+                                          const uint32_t *__restrict__ list_len,
                                           float4 *__restrict__ force, const LvPair *s_pair)
 {
     constexpr int T = 32 / S;
@@ -884,7 +907,7 @@ __device__ __forceinline__ void rows_body(const LvDev &P, const float4 *__restri
         const float4 pi = pos[self];
         const LvPair *pair_a = s_pair + (live ? __float_as_int(pi.w) : 0) * LV_MAX_TYPES;
         const uint32_t b0 = live ? __ldg(list_start + i) : 0u;
-        const uint32_t len = live ? __ldg(list_start + i + 1) - b0 : 0u;     // a multiple of 4
+        const uint32_t len = live ? __ldg(list_len + i) : 0u;                // a multiple of 4
         const uint32_t maxlen = __reduce_max_sync(kFull, len);
         const uint32_t *lp = list + b0 + ls;
         float fx = 0.f, fy = 0.f, fz = 0.f;
@@ -943,8 +966,8 @@ template <bool kCharged>
 __global__ void __launch_bounds__(kRThreads)
 k_pair_force_rows(const __grid_constant__ LvDev P, const float4 *__restrict__ posA,
                   const float4 *__restrict__ posB, const uint32_t *__restrict__ list,
-                  const uint32_t *__restrict__ list_start, float4 *__restrict__ force,
-                  const LvDevState *st)
+                  const uint32_t *__restrict__ list_start, const uint32_t *__restrict__ list_len,
+                  float4 *__restrict__ force, const LvDevState *st)
 {
     if (st->list_ok == 0u) return;          // the cell kernel takes this step
     __shared__ LvPair s_pair[LV_MAX_TYPES * LV_MAX_TYPES];
@@ -952,25 +975,56 @@ k_pair_force_rows(const __grid_constant__ LvDev P, const float4 *__restrict__ po
     __syncthreads();
     const float4 *__restrict__ pos = st->rebuild[st->step & 1] ? posB : posA;
     const unsigned int S = P.list_lanes_forced ? (unsigned int)P.list_lanes_forced : st->list_lanes;
-    if (S == 1u) rows_body<kCharged, 1>(P, pos, list, list_start, force, s_pair);
-    else if (S == 2u) rows_body<kCharged, 2>(P, pos, list, list_start, force, s_pair);
-    else if (S == 4u) rows_body<kCharged, 4>(P, pos, list, list_start, force, s_pair);
-    else if (S == 8u) rows_body<kCharged, 8>(P, pos, list, list_start, force, s_pair);
-    else if (S == 16u) rows_body<kCharged, 16>(P, pos, list, list_start, force, s_pair);
-    else rows_body<kCharged, 32>(P, pos, list, list_start, force, s_pair);
+    if (S == 1u) rows_body<kCharged, 1>(P, pos, list, list_start, list_len, force, s_pair);
+    else if (S == 2u) rows_body<kCharged, 2>(P, pos, list, list_start, list_len, force, s_pair);
+    else if (S == 4u) rows_body<kCharged, 4>(P, pos, list, list_start, list_len, force, s_pair);
+    else if (S == 8u) rows_body<kCharged, 8>(P, pos, list, list_start, list_len, force, s_pair);
+    else if (S == 16u) rows_body<kCharged, 16>(P, pos, list, list_start, list_len, force, s_pair);
+    else rows_body<kCharged, 32>(P, pos, list, list_start, list_len, force, s_pair);
 }
 
-// After the count pass and the scan of the lengths: does the list fit its pool, and how many
-// lanes share an NP's list (from the mean length, so the choice is a function of the state).
-__global__ void k_list_check(int n, uint32_t pool, LvDevState *st)
+// One-walk build, step 1: reserve for every NP its previous length + 1/8 + 32 entries (lists
+// change little between two rebuilds), in the NEW slot order (perm[i] = slot of the previous
+// order).  Without a valid previous list the exact two-pass build is switched on instead.
+__global__ void __launch_bounds__(kThreads)
+k_list_reserve(int n, uint32_t n_tiles, const uint32_t *__restrict__ perm, const uint32_t *__restrict__ len_prev,
+               uint32_t *__restrict__ cnt, unsigned long long *__restrict__ scan_tile,
+               unsigned int *__restrict__ scan_ticket, LvDevState *st)
 {
     if (skipped(st)) return;
+    const int i = blockIdx.x * kThreads + threadIdx.x;
+    // ... also while the lists are short (mean below 128 entries): there the reserve's gaps cost
+    // the force kernel more (the list spreads over twice the memory) than the second walk costs
+    if (st->list_prev == 0u || st->list_ok == 0u || st->list_used < 128ull * (unsigned long long)n) {
+        if (i == 0) st->list_redo = 1u;
+        return;
+    }
+    if (i < (int)n_tiles) scan_tile[i] = 0ull;          // re-arm the scan of the reserves
+    if (i == 0) { *scan_ticket = 0u; cnt[n] = 0u; }
+    uint32_t cap = 0u;
+    if (i < n) {
+        const uint32_t L = len_prev[perm[i]];
+        cap = (L + (L >> 3) + 32u + 3u) & ~3u;
+        cnt[i] = cap;
+    }
+    const uint32_t wsum = __reduce_add_sync(kFull, cap);
+    if ((threadIdx.x & 31) == 0 && wsum) atomicAdd(&st->list_total, (unsigned long long)wsum);
+}
+
+// After the reserve / count pass and the scan: does the list fit its pool, and how many lanes
+// share an NP's list (from the mean length, so the choice is a function of the state).
+// exact = false: the one-walk build (a reserve that does not fit hands over to the exact build).
+__global__ void k_list_check(int n, uint32_t pool, bool exact, LvDevState *st)
+{
+    if (skipped(st)) return;
+    if (exact != (st->list_redo != 0u)) return;
     if (st->list_ok == 0u && ((st->step & 63) != 0 || st->list_defer != 0u)) return;   // not counted this step
     const unsigned long long total = st->list_total;
+    st->list_total = 0ull;
     const bool fits = total <= (unsigned long long)pool;
+    if (!exact && !fits) { st->list_redo = 1u; return; }
     st->list_ok = fits ? 1u : 0u;
     st->list_used = total;
-    st->list_total = 0ull;
     const unsigned long long mean = total / (unsigned long long)(n > 0 ? n : 1);
     st->list_lanes = mean < 64ull ? 4u : 8u;          // measured on C3
     if (!fits) atomicOr(&st->status, LV_ST_LIST_OVERFLOW);
@@ -1037,7 +1091,13 @@ k_update(const __grid_constant__ LvDev P, const float4 *__restrict__ posB_,
             st->ticket = 0u;
             st->step = n0 + 1;
             if (kList) {
+                if (st->rebuild[n0 & 1] != 0u && st->list_ok != 0u) {     // a list was built
+                    st->n_rebuilds += 1u;
+                    if (st->list_redo != 0u) st->n_exact += 1u;           // ... by the two-pass build
+                }
                 st->rebuild[n0 & 1] = 0u;              // ... and this step's rebuild flag
+                st->list_redo = 0u;
+                st->list_prev = st->list_ok;           // list_len[] describes a list in the present slot order
                 if (st->list_ok == 0u) {               // on the cell kernel: every step rebuilds the cells
                     st->rebuild[(n0 + 1) & 1] = 1u;
                     if (st->list_defer != 0u) {        // first step after lv_set_state: the next one builds the list
@@ -1141,11 +1201,14 @@ k_pack_state(int n, int n_types, const float *__restrict__ pos, const float *__r
         st->rebuild[(step + 1) & 1] = 0u;
         st->n_rebuilds = 0u;
         st->list_ok = 0u;
+        st->list_prev = 0u;
+        st->list_redo = 0u;
         st->list_defer = 1u;
         st->list_lanes = 8u;
         st->list_total = 0ull;
         st->list_used = 0ull;
         st->n_fallback = 0u;
+        st->n_exact = 0u;
     }
     if (i >= n) return;
     int a = type[i];
@@ -1640,36 +1703,57 @@ cudaError_t lvk_pair_force(const LvDev &P, const LvBufs &B, int variant, cudaStr
         if (variant == 3) {
             if (charged)
                 k_pair_force_s<true, 1><<<blocks, kSThreads, 0, st>>>(P, B.posB, B.cell_off, B.force,
-                                                                      B.posP, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr);
+                                                                      B.posP, LvListArgs{}, nullptr);
             else
                 k_pair_force_s<false, 1><<<blocks, kSThreads, 0, st>>>(P, B.posB, B.cell_off, B.force,
-                                                                       B.posP, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr);
+                                                                       B.posP, LvListArgs{}, nullptr);
         } else {
             if (charged)
                 k_pair_force_s<true, 0><<<blocks, kSThreads, 0, st>>>(P, B.posB, B.cell_off, B.force,
-                                                                      nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr);
+                                                                      nullptr, LvListArgs{}, nullptr);
             else
                 k_pair_force_s<false, 0><<<blocks, kSThreads, 0, st>>>(P, B.posB, B.cell_off, B.force,
-                                                                       nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr);
+                                                                       nullptr, LvListArgs{}, nullptr);
         }
     }
     return cudaGetLastError();
 }
 
-// skin list: count the (padded) list lengths, scan them into the list starts, check the pool,
-// fill -- all guarded by this step's rebuild flag
+// First node of a list step's graph: hands this step's rebuild flag to the IF node that holds
+// the whole rebuild chain (a guarded kernel that returns at once still costs ~1.5 us of a
+// graph replay; the chain has thirteen of them).
+namespace {
+__global__ void k_list_cond(cudaGraphConditionalHandle h, const LvDevState *st)
+{
+    if (threadIdx.x == 0) cudaGraphSetConditional(h, st->rebuild[st->step & 1] != 0u ? 1u : 0u);
+}
+}  // namespace
+
+cudaError_t lvk_list_cond(unsigned long long handle, const LvBufs &B, cudaStream_t st)
+{
+    k_list_cond<<<1, 32, 0, st>>>((cudaGraphConditionalHandle)handle, B.st);
+    return cudaGetLastError();
+}
+
+// skin list build, all kernels guarded by this step's rebuild flag.  One-walk build: reserve
+// from the previous lengths, scan, pool check, fill.  Exact build (first list, after a fallback,
+// or when a list outgrew its reserve: list_redo): count, scan, pool check, fill.
 cudaError_t lvk_list_build(const LvDev &P, const LvBufs &B, cudaStream_t st)
 {
     const int m = P.n > (int)P.n_list_tiles ? P.n : (int)P.n_list_tiles;
-    const int blocks = (m + kSThreads - 1) / kSThreads;
-    k_pair_force_s<false, 3><<<blocks, kSThreads, 0, st>>>(P, B.posB, B.cell_off, nullptr, nullptr, nullptr,
-                                                           B.list_cnt, nullptr, B.list_scan_tile,
-                                                           B.list_scan_ticket, B.st);
+    const int blocks = (m + kSThreads - 1) / kSThreads, fblocks = (P.n + kSThreads - 1) / kSThreads;
+    const LvListArgs LA = {B.list, B.list_cnt, B.list_start, B.list_len, B.list_scan_tile, B.list_scan_ticket};
+    k_list_reserve<<<blocks_for(m), kThreads, 0, st>>>(P.n, P.n_list_tiles, B.val_out, B.list_len, B.list_cnt,
+                                                       B.list_scan_tile, B.list_scan_ticket, B.st);
     k_scan_cells<<<P.n_list_tiles, kScanThreads, 0, st>>>((uint32_t)P.n + 1u, B.list_cnt, B.list_start,
-                                                          B.list_scan_tile, B.list_scan_ticket, B.st, B.st);
-    k_list_check<<<1, 1, 0, st>>>(P.n, P.list_pool, B.st);
-    k_pair_force_s<false, 2><<<(P.n + kSThreads - 1) / kSThreads, kSThreads, 0, st>>>(
-        P, B.posB, B.cell_off, nullptr, nullptr, B.list, nullptr, B.list_start, nullptr, nullptr, B.st);
+                                                          B.list_scan_tile, B.list_scan_ticket, B.st, B.st, 1);
+    k_list_check<<<1, 1, 0, st>>>(P.n, P.list_pool, false, B.st);
+    k_pair_force_s<false, 4><<<fblocks, kSThreads, 0, st>>>(P, B.posB, B.cell_off, nullptr, nullptr, LA, B.st);
+    k_pair_force_s<false, 3><<<blocks, kSThreads, 0, st>>>(P, B.posB, B.cell_off, nullptr, nullptr, LA, B.st);
+    k_scan_cells<<<P.n_list_tiles, kScanThreads, 0, st>>>((uint32_t)P.n + 1u, B.list_cnt, B.list_start,
+                                                          B.list_scan_tile, B.list_scan_ticket, B.st, B.st, 2);
+    k_list_check<<<1, 1, 0, st>>>(P.n, P.list_pool, true, B.st);
+    k_pair_force_s<false, 2><<<fblocks, kSThreads, 0, st>>>(P, B.posB, B.cell_off, nullptr, nullptr, LA, B.st);
     return cudaGetLastError();
 }
 
@@ -1679,10 +1763,10 @@ cudaError_t lvk_pair_force_list(const LvDev &P, const LvBufs &B, cudaStream_t st
     const int blocks = (P.n + per_block - 1) / per_block;
     if (lvk_any_charge(P))
         k_pair_force_rows<true><<<blocks, kRThreads, 0, st>>>(P, B.posA, B.posB, B.list, B.list_start,
-                                                              B.force, B.st);
+                                                              B.list_len, B.force, B.st);
     else
         k_pair_force_rows<false><<<blocks, kRThreads, 0, st>>>(P, B.posA, B.posB, B.list, B.list_start,
-                                                               B.force, B.st);
+                                                               B.list_len, B.force, B.st);
     return cudaGetLastError();
 }
 
@@ -1690,11 +1774,11 @@ cudaError_t lvk_pair_force_fallback(const LvDev &P, const LvBufs &B, cudaStream_
 {
     const int blocks = (P.n + kSThreads - 1) / kSThreads;
     if (lvk_any_charge(P))
-        k_pair_force_s<true, 0><<<blocks, kSThreads, 0, st>>>(P, B.posB, B.cell_off, B.force, nullptr, nullptr,
-                                                              nullptr, nullptr, nullptr, nullptr, B.st);
+        k_pair_force_s<true, 0><<<blocks, kSThreads, 0, st>>>(P, B.posB, B.cell_off, B.force, nullptr,
+                                                              LvListArgs{}, B.st);
     else
-        k_pair_force_s<false, 0><<<blocks, kSThreads, 0, st>>>(P, B.posB, B.cell_off, B.force, nullptr, nullptr,
-                                                               nullptr, nullptr, nullptr, nullptr, B.st);
+        k_pair_force_s<false, 0><<<blocks, kSThreads, 0, st>>>(P, B.posB, B.cell_off, B.force, nullptr,
+                                                               LvListArgs{}, B.st);
     return cudaGetLastError();
 }
 
@@ -1711,7 +1795,7 @@ cudaError_t lvk_scan_cells(const LvDev &P, const LvBufs &B, bool guarded, cudaSt
 {
     k_scan_cells<<<P.n_scan_tiles, kScanThreads, 0, st>>>(P.n_cells + 1u, B.cell_cnt, B.cell_off,
                                                           B.scan_tile, B.scan_ticket,
-                                                          guarded ? B.st : nullptr, nullptr);
+                                                          guarded ? B.st : nullptr, nullptr, 0);
     return cudaGetLastError();
 }
 
