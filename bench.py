@@ -231,7 +231,7 @@ def make_sim(binding, w, args, device, cpc=None, use_list=None):
         cpc = args.cells_per_cut if args.cells_per_cut else w.tuned_cells_per_cut
     if use_list is None:
         use_list = not args.no_list and args.force_kernel in (None, 2)
-    nl = (args.skin, -1) if use_list else None
+    nl = (args.skin, -1) if use_list else None      # from_workload's own default is (0, -1) too
     return binding.Simulation.from_workload(w, cells_per_cut=cpc, device=device, options=options or None,
                                             neighbour_list=nl), cpc, use_list
 

@@ -362,10 +362,12 @@ class Simulation:
         v.background, v.droplet = int(background), int(droplet)
         with torch.cuda.device(self.device):
             n_px = int(width) * int(height)
-            # depth keys (8 B per pixel) + the staged image for host output (4 B per pixel)
-            zbuf = torch.empty(n_px + (0 if on_device else (n_px + 1) // 2), dtype=torch.int64,
-                               device=self.device)
-            zbuf.record_stream(self.stream)
+            # depth keys (8 B per pixel) + the staged image for host output (4 B per pixel); kept
+            # between calls (a fresh allocation per frame costs more than the frame)
+            need = n_px + (n_px + 1) // 2
+            zbuf = getattr(self, "_view_scratch", None)
+            if zbuf is None or zbuf.numel() < need:
+                zbuf = self._view_scratch = torch.empty(need, dtype=torch.int64, device=self.device)
             if on_device:
                 img = torch.empty((int(height), int(width)), dtype=torch.int32, device=self.device)
                 img.record_stream(self.stream)
@@ -388,9 +390,10 @@ class Simulation:
         m.droplet = int(droplet)
         w_, h_ = max(int(width), 0), max(int(height), 0)
         with torch.cuda.device(self.device):
-            scratch = torch.empty(w_ * h_ + w_ + h_ + 1 + (0 if on_device else (w_ * h_ + 1) // 2),
-                                  dtype=torch.int64, device=self.device)
-            scratch.record_stream(self.stream)
+            need = w_ * h_ + w_ + h_ + 1 + (w_ * h_ + 1) // 2
+            scratch = getattr(self, "_view_scratch", None)
+            if scratch is None or scratch.numel() < need:
+                scratch = self._view_scratch = torch.empty(need, dtype=torch.int64, device=self.device)
             if on_device:
                 img = torch.empty((h_, w_), dtype=torch.int32, device=self.device)
                 img.record_stream(self.stream)
@@ -462,6 +465,7 @@ class Simulation:
             self.L.lv_destroy(self.h)
             self.h = C.c_void_p()
         self.workspace = None
+        self._view_scratch = None
 
     def __del__(self):
         try:
@@ -472,9 +476,13 @@ class Simulation:
     # -- convenience -----------------------------------------------------------
     @classmethod
     def from_workload(cls, w, cells_per_cut=None, device="cuda:0", load_state=True,
-                      options=None, neighbour_list=None) -> "Simulation":
+                      options=None, neighbour_list="auto") -> "Simulation":
         """Configure from a workloads.Workload: per-type (a, b) through
-        lv_langevin_coeffs, Lorentz-Berthelot tables inside lv_set_types."""
+        lv_langevin_coeffs, Lorentz-Berthelot tables inside lv_set_types.
+        neighbour_list: "auto" (default) = lv_set_neighbour_list(skin <= 0, -1), the product path
+        (automatic skin and pool; the library keeps the cells below 16 384 NPs) -- unless
+        `options` choose the radix sort or another force kernel than the default, which are
+        cell-path choices; None = off (cells rebuilt every step); or (skin, capacity)."""
         sim = cls(w.n, w.n_types, w.seed, w.dt, device=device)
         types = []
         for a in range(w.n_types):
@@ -488,6 +496,12 @@ class Simulation:
             sim.set_grid(cells_per_cut)
         for opt, val in (options or {}).items():
             sim.set_option(opt, val)
+        if isinstance(neighbour_list, str):
+            assert neighbour_list == "auto"
+            o = options or {}
+            cell_choice = (o.get(OPT_SORT, SORT_COUNTING) != SORT_COUNTING
+                           or o.get(OPT_FORCE_KERNEL, FORCE_SEGMENTS) != FORCE_SEGMENTS)
+            neighbour_list = None if cell_choice else (0.0, -1)
         if neighbour_list is not None:          # (skin, capacity)
             sim.set_neighbour_list(*neighbour_list)
         sim.bind()

@@ -67,7 +67,7 @@ def test_list_stays_complete_between_rebuilds(B, name, n, cpc, skin, cap):
     the same state: no in-range pair is ever missing from a list that was built steps ago."""
     w = W.make_workload(name, n)
     lst = B.Simulation.from_workload(w, cells_per_cut=cpc, neighbour_list=(skin, cap))
-    cel = B.Simulation.from_workload(w, cells_per_cut=cpc)
+    cel = B.Simulation.from_workload(w, cells_per_cut=cpc, neighbour_list=None)
     done = 0
     for k in (3, 37, 150, 400):
         lst.step(k - done)
@@ -138,7 +138,7 @@ def test_pool_too_small_falls_back_to_the_cells(B):
     path, so counts, forces and the trajectory are BIT-identical to a run without the list."""
     w = W.make_workload("C4", 19999)              # ~50 neighbours per NP
     lst = B.Simulation.from_workload(w, cells_per_cut=[2], neighbour_list=(0.2, 8))
-    cel = B.Simulation.from_workload(w, cells_per_cut=[2])
+    cel = B.Simulation.from_workload(w, cells_per_cut=[2], neighbour_list=None)
     lst.step(1); cel.step(1)
     Fl, cl = lst.get_forces()
     Fc, cc = cel.get_forces()
@@ -174,7 +174,7 @@ def test_list_follows_a_shrinking_droplet_into_the_fallback(B, orc):
     st = a.list_stats()
     assert 0 < st["fallback_steps"] < 7000 and st["rebuilds"] > 1
     assert a.status() & B.ST_LIST_OVERFLOW
-    cel = B.Simulation.from_workload(w, cells_per_cut=[2, 2], load_state=False)
+    cel = B.Simulation.from_workload(w, cells_per_cut=[2, 2], load_state=False, neighbour_list=None)
     cel.set_state(xa, va, ta, sa)
     cel.compute_forces()
     Fc, cc = cel.get_forces()

@@ -246,7 +246,7 @@ def test_steady_state_permutation_against_the_oracle(B, orc, name, n, cpc):
     w = workload(name, n)
     p = orc.params_from_workload(w)
     g = orc.grid_spec(p, cpc)
-    sim = B.Simulation.from_workload(w, cells_per_cut=cpc)
+    sim = B.Simulation.from_workload(w, cells_per_cut=cpc, neighbour_list=None)    # the cells, every step
     sim.step(5)
     ids_prev = sim.get_debug(B.DBG_IDS_SORTED).astype(np.int64)
     moved = 0
@@ -714,7 +714,7 @@ def test_implementation_options_do_not_change_results(B, orc, name, n, cpc):
     g = orc.grid_spec(p, cpc)
     key, ks, perm, off = orc.cell_structures(g, w.pos, w.type)
     Fo, So, co, _ = orc.pair_forces(p, w.pos, w.type, "cells")
-    ref = B.Simulation.from_workload(w, cells_per_cut=cpc)
+    ref = B.Simulation.from_workload(w, cells_per_cut=cpc, neighbour_list=None)
     ref.compute_forces()
     F0, c0 = ref.get_forces()
     ref.step(30)
