@@ -89,6 +89,7 @@ struct LvDevState {
     unsigned int list_redo;
     unsigned int n_exact;          // rebuilds done by the exact two-pass build since lv_set_state
     unsigned int pad;
+    unsigned long long list_true;  // true (padded) entries of the list being filled / last filled
 };
 
 struct LvBufs {

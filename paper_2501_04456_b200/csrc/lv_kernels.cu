@@ -863,7 +863,10 @@ k_pair_force_s(const __grid_constant__ LvDev P, const float4 *__restrict__ pos,
                 ebuf.w = self;
                 col[cnt >> 2] = ebuf;
             }
-            if (live) LA.len[i] = ((uint32_t)cnt + 3u) & ~3u;
+            const uint32_t tlen = live ? ((uint32_t)cnt + 3u) & ~3u : 0u;
+            if (live) LA.len[i] = tlen;
+            const uint32_t tsum = __reduce_add_sync(kFull, tlen);
+            if ((gtid & 31) == 0 && tsum) atomicAdd(&st->list_true, (unsigned long long)tsum);
             // one-walk build: a list that outgrew its reserve hands the rebuild to the exact build
             if (kOpt && live && cnt > cap) st->list_redo = 1u;
         }
@@ -881,6 +884,9 @@ k_pair_force_s(const __grid_constant__ LvDev P, const float4 *__restrict__ pos,
 // list length (LvDevState::list_lanes: 4 below 64 entries, else 8; LV_OPT_LIST_LANES forces it).
 // The positions are those of the list's slot order: posB on the step that rebuilt, else posA
 // (k_update keeps that order until the next rebuild).
+#ifndef LV_LIST_MARGIN
+#define LV_LIST_MARGIN 16u
+#endif
 constexpr int kRThreads = 128;
 constexpr int kRPerWarp = 8;        // NPs per warp: small work items, balanced by the block scheduler
 
@@ -983,7 +989,7 @@ k_pair_force_rows(const __grid_constant__ LvDev P, const float4 *__restrict__ po
     else rows_body<kCharged, 32>(P, pos, list, list_start, list_len, force, s_pair);
 }
 
-// One-walk build, step 1: reserve for every NP its previous length + 1/8 + 32 entries (lists
+// One-walk build, step 1: reserve for every NP its previous length + 1/8 + 16 entries (lists
 // change little between two rebuilds), in the NEW slot order (perm[i] = slot of the previous
 // order).  Without a valid previous list the exact two-pass build is switched on instead.
 __global__ void __launch_bounds__(kThreads)
@@ -993,9 +999,7 @@ k_list_reserve(int n, uint32_t n_tiles, const uint32_t *__restrict__ perm, const
 {
     if (skipped(st)) return;
     const int i = blockIdx.x * kThreads + threadIdx.x;
-    // ... also while the lists are short (mean below 128 entries): there the reserve's gaps cost
-    // the force kernel more (the list spreads over twice the memory) than the second walk costs
-    if (st->list_prev == 0u || st->list_ok == 0u || st->list_used < 128ull * (unsigned long long)n) {
+    if (st->list_prev == 0u || st->list_ok == 0u) {
         if (i == 0) st->list_redo = 1u;
         return;
     }
@@ -1004,7 +1008,7 @@ k_list_reserve(int n, uint32_t n_tiles, const uint32_t *__restrict__ perm, const
     uint32_t cap = 0u;
     if (i < n) {
         const uint32_t L = len_prev[perm[i]];
-        cap = (L + (L >> 3) + 32u + 3u) & ~3u;
+        cap = (L + (L >> 3) + LV_LIST_MARGIN + 3u) & ~3u;
         cnt[i] = cap;
     }
     const uint32_t wsum = __reduce_add_sync(kFull, cap);
@@ -1025,8 +1029,11 @@ __global__ void k_list_check(int n, uint32_t pool, bool exact, LvDevState *st)
     if (!exact && !fits) { st->list_redo = 1u; return; }
     st->list_ok = fits ? 1u : 0u;
     st->list_used = total;
-    const unsigned long long mean = total / (unsigned long long)(n > 0 ? n : 1);
+    // lanes per NP from the mean TRUE length: the count itself (exact build) or the previous
+    // list's (one-walk build: its reserve is ~1.5 x the length for short lists)
+    const unsigned long long mean = (exact ? total : st->list_true) / (unsigned long long)(n > 0 ? n : 1);
     st->list_lanes = mean < 64ull ? 4u : 8u;          // measured on C3
+    st->list_true = 0ull;                             // the fill that follows sums the new one
     if (!fits) atomicOr(&st->status, LV_ST_LIST_OVERFLOW);
 }
 
@@ -1209,6 +1216,7 @@ k_pack_state(int n, int n_types, const float *__restrict__ pos, const float *__r
         st->list_used = 0ull;
         st->n_fallback = 0u;
         st->n_exact = 0u;
+        st->list_true = 0ull;
     }
     if (i >= n) return;
     int a = type[i];
