@@ -99,6 +99,8 @@ def lib():
         L.lvo_render.argtypes = [C.c_int, fp, ip, fp, fp, C.c_float, C.c_float, C.c_int, C.c_int, up,
                                  C.c_uint32, C.c_uint32, C.c_float, up]
         L.lvo_render.restype = None
+        L.lvo_render_pixels.argtypes = L.lvo_render.argtypes
+        L.lvo_render_pixels.restype = None
         L.lvo_render_surface.argtypes = [C.c_int, fp, ip, fp, C.c_float, C.c_int, C.c_int, up,
                                          C.c_uint32, up]
         L.lvo_render_surface.restype = None
@@ -354,8 +356,9 @@ def view_rotation(yaw, pitch):
 
 
 def render(x_f32, type_, radius_a, R, eye_dist, focal_px, yaw, pitch, width, height, palette,
-           background, droplet):
-    """Perspective splat of Fig. 2 (right panel) -> uint32[height, width] (0xAABBGGRR)."""
+           background, droplet, per_pixel=False):
+    """Perspective splat of Fig. 2 (right panel) -> uint32[height, width] (0xAABBGGRR).
+    per_pixel: the definition written out -- every pixel against every NP (small frames)."""
     x = np.ascontiguousarray(x_f32, dtype=np.float32).reshape(-1, 3)
     t = _ci32(type_)
     ra = np.ascontiguousarray(radius_a, dtype=np.float32)
@@ -363,7 +366,8 @@ def render(x_f32, type_, radius_a, R, eye_dist, focal_px, yaw, pitch, width, hei
     pal[:len(palette)] = np.asarray(palette, dtype=np.uint32)
     rot = view_rotation(yaw, pitch)
     img = np.zeros((int(height), int(width)), dtype=np.uint32)
-    lib().lvo_render(x.shape[0], _f(x), _i(t), _f(ra), _f(rot), C.c_float(float(np.float32(eye_dist))),
+    fn = lib().lvo_render_pixels if per_pixel else lib().lvo_render
+    fn(x.shape[0], _f(x), _i(t), _f(ra), _f(rot), C.c_float(float(np.float32(eye_dist))),
                      C.c_float(float(np.float32(focal_px))), int(width), int(height), _u(pal),
                      int(background), int(droplet), C.c_float(float(np.float32(R))), _u(img))
     return img

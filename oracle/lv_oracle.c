@@ -671,6 +671,53 @@ void lvo_render(int n, const float *x, const int32_t *type, const float *radius_
     free(zb);
 }
 
+/* The same view written as its DEFINITION, pixel by pixel: for EVERY pixel, EVERY NP is projected
+ * and tested -- no bounding boxes, no per-NP pixel loops -- and the nearest fragment is kept.
+ * O(pixels x NPs): small frames only.  lvo_render (the per-NP form the CUDA splat mirrors) must
+ * give the same image bit for bit; a mistake in its bounding-box logic cannot hide here. */
+void lvo_render_pixels(int n, const float *x, const int32_t *type, const float *radius_a,
+                       const float *rot, float eye, float focal, int width, int height,
+                       const uint32_t *palette, uint32_t background, uint32_t droplet, float R,
+                       uint32_t *rgba)
+{
+    float cx = (float)(0.5 * width), cy = (float)(0.5 * height);
+    float rr = R * (focal / eye);
+#pragma omp parallel for schedule(static)
+    for (int py = 0; py < height; ++py)
+        for (int px = 0; px < width; ++px) {
+            uint64_t best = ~(uint64_t)0;
+            for (int i = 0; i < n; ++i) {
+                float px_ = x[3 * i], py_ = x[3 * i + 1], pz_ = x[3 * i + 2];
+                float r = radius_a[type[i]];
+                float xc = (rot[0] * px_ + rot[1] * py_) + rot[2] * pz_;
+                float yc = (rot[3] * px_ + rot[4] * py_) + rot[5] * pz_;
+                float zr = (rot[6] * px_ + rot[7] * py_) + rot[8] * pz_;
+                float zc = eye - zr;
+                if (!(zc > 2.0f * r)) continue;
+                float inv = focal / zc;
+                float u = cx + xc * inv;
+                float v = cy - yc * inv;
+                float rho = r * inv;
+                float rho2 = rho * rho;
+                if (!(rho2 > 0.0f) || !(fabsf(u) < 1e7f) || !(fabsf(v) < 1e7f) || !(rho < 1e4f)) continue;
+                float dx = ((float)px + 0.5f) - u, dy = ((float)py + 0.5f) - v;
+                float d2 = dx * dx + dy * dy;
+                if (!(d2 <= rho2)) continue;
+                float nz = sqrtf((rho2 - d2) / rho2);
+                float zf = zc - r * nz;
+                uint32_t c = shade_px(palette[type[i]], 0.25f + 0.75f * nz);
+                uint32_t zbits;
+                memcpy(&zbits, &zf, 4);
+                uint64_t key = ((uint64_t)zbits << 32) | c;
+                if (key < best) best = key;
+            }
+            size_t p = (size_t)py * width + px;
+            if (best != ~(uint64_t)0) { rgba[p] = (uint32_t)best; continue; }
+            float dx = ((float)px + 0.5f) - cx, dy = ((float)py + 0.5f) - cy;
+            rgba[p] = dx * dx + dy * dy <= rr * rr ? droplet : background;
+        }
+}
+
 /* Surface map, the left panel of Fig. 2 ("projection of the microdroplet
  * surface onto a plane", NP intersections with the surface as circles "elongated due to the
  * projection"); the projection is this build's reading (equirectangular, pole = z), its

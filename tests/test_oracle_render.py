@@ -70,3 +70,28 @@ def test_rotation_orientation():
     x0 = np.nonzero((im0 != BG) & (im0 != DROP))[1].mean()
     x1 = np.nonzero((im1 != BG) & (im1 != DROP))[1].mean()
     assert abs(x0 - 100.0) < 0.6 and abs(x1 - (100.5 + 40.0 - 0.5)) < 0.6
+
+
+def test_per_np_splat_equals_the_per_pixel_definition():
+    """lvo_render walks, per NP, the bounding box of its projected disc (the structure the CUDA
+    splat mirrors); lvo_render_pixels is the definition -- every pixel against every NP, no
+    boxes.  Bit-identical images on crowded, clipped, close-up and inside-the-droplet scenes pin
+    the bounding-box logic to something that does not share it."""
+    rng = np.random.default_rng(7)
+    pal = [0x00ff8040, 0x004080ff, 0x0040ff80]
+    for n, R, eye, focal, yaw, pitch, W, H in (
+            (400, 10.0, 30.0, 120.0, 0.3, -0.2, 96, 64),        # the whole droplet
+            (400, 10.0, 12.0, 200.0, 1.1, 0.4, 77, 53),         # close: discs clipped by the frame
+            (300, 10.0, 4.0, 60.0, -0.7, 0.9, 64, 48),          # camera INSIDE: NPs behind / around it
+            (50, 3.0, 500.0, 40.0, 0.0, 0.0, 33, 31),           # far: sub-pixel discs
+            (0, 5.0, 20.0, 50.0, 0.0, 0.0, 16, 9)):             # empty
+        x = rng.normal(0, 1, size=(n, 3))
+        x *= (R * rng.random(n) ** (1 / 3) / np.maximum(np.linalg.norm(x, axis=1), 1e-9))[:, None]
+        t = rng.integers(0, 3, size=n).astype(np.int32)
+        ra = [0.4, 0.7, 1.3]
+        a = oracle.render(x.astype(np.float32), t, ra, R, eye, focal, yaw, pitch, W, H, pal, BG, DROP)
+        b = oracle.render(x.astype(np.float32), t, ra, R, eye, focal, yaw, pitch, W, H, pal, BG, DROP,
+                          per_pixel=True)
+        assert np.array_equal(a, b)
+        if n:
+            assert ((a != BG) & (a != DROP)).any()
