@@ -49,7 +49,7 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
-from paper_2501_04456_b200 import replicas, workloads  # noqa: E402
+from paper_2501_04456_b200 import replicas, tuning, workloads  # noqa: E402
 
 METRIC = "particle-steps/sec at N=2.5e5"
 UNIT = "particle-steps/s"
@@ -228,7 +228,7 @@ def make_sim(binding, w, args, device, cpc=None, use_list=None):
     if args.tile_substreams is not None:
         options[binding.OPT_TILE_SUBSTREAMS] = args.tile_substreams
     if cpc is None:
-        cpc = args.cells_per_cut if args.cells_per_cut else w.tuned_cells_per_cut
+        cpc = args.cells_per_cut if args.cells_per_cut else tuning.cells_per_cut(w)
     if use_list is None:
         use_list = not args.no_list and args.force_kernel in (None, 2)
     nl = (args.skin, -1) if use_list else None      # from_workload's own default is (0, -1) too

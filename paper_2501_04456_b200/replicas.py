@@ -77,13 +77,13 @@ class ReplicaSet:
                  cells_per_cut=None, options=None, neighbour_list=None, slice_steps: int = 50,
                  batched: bool = True, steps_per_launch: int = 8):
         _check_cuda_extension()
-        from . import binding
+        from . import binding, tuning
         if n_replicas < 1:
             raise ValueError("n_replicas must be >= 1")
         self.slice_steps = int(slice_steps)
         self.workloads = [make_workload(replica_seed(base_seed, r)) for r in range(n_replicas)]
         self.sims = [binding.Simulation.from_workload(
-            w, cells_per_cut=cells_per_cut if cells_per_cut is not None else w.tuned_cells_per_cut,
+            w, cells_per_cut=cells_per_cut if cells_per_cut is not None else tuning.cells_per_cut(w),
             device=device, options=options, neighbour_list=neighbour_list) for w in self.workloads]
         self.batch = binding.Batch(self.sims, steps_per_launch) if batched else None
 

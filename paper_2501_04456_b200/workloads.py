@@ -56,12 +56,6 @@ class Workload:
     steps: int
     init: str                   # "ball" | "fcc"
     eps_matrix: Optional[np.ndarray] = None
-    # cells per cut-off per type (lv_set_grid) measured fastest on B200 for this config
-    # (DESIGN.md sec. 7.2); bench.py's default.  A tuning choice, not part of the model.
-    tuned_cells_per_cut: Optional[List[int]] = None
-    # (skin, entries per NP) for lv_set_neighbour_list at the START of the schedule, used by
-    # bench.py's skin-list variant; a shrinking droplet needs more capacity later on
-    tuned_neighbour_list: Optional[Sequence[float]] = None
     pos: np.ndarray = field(default=None, repr=False)    # [n,3] float32
     vel: np.ndarray = field(default=None, repr=False)    # [n,3] float32
     type: np.ndarray = field(default=None, repr=False)   # [n] int32
@@ -83,16 +77,14 @@ def _spec(name: str) -> Workload:
                         kT=1.0, dt=0.005, cut_factor=2.5, coulomb_k=0.0, g=0.0,
                         omega2=(0.0, 0.0, 0.0), wall_mode=WALL_ONESIDED,
                         sched_mode=SCHED_CONST, R0=20.0, R1=20.0, sched_steps=0,
-                        seed=1, steps=1000, init="ball", tuned_cells_per_cut=[1],
-                        tuned_neighbour_list=(0.3, 64))
+                        seed=1, steps=1000, init="ball")
     if name == "C2":
         s = [1.0, 1.5]
         return Workload("C2", 32768, s, [1.0, 2.0], [1.0, -1.0], _mass(s), [100.0] * 2,
                         [1.0] * 2, [0.7, 0.3], kT=1.0, dt=0.002, cut_factor=5.0,
                         coulomb_k=0.7, g=0.0, omega2=(0.0, 0.0, 0.0),
                         wall_mode=WALL_ONESIDED, sched_mode=SCHED_LINEAR, R0=60.0, R1=25.0,
-                        sched_steps=10000, seed=2, steps=10000, init="ball", tuned_cells_per_cut=[2, 2],
-                        tuned_neighbour_list=(0.4, 256))
+                        sched_steps=10000, seed=2, steps=10000, init="ball")
     if name == "C3":
         s = [1.0, 1.5, 2.5]
         w2 = 0.005 ** 2
@@ -100,8 +92,7 @@ def _spec(name: str) -> Workload:
                         [100.0] * 3, [2.0] * 3, [0.5, 0.3, 0.2], kT=1.0, dt=0.002,
                         cut_factor=5.0, coulomb_k=0.7, g=0.01, omega2=(w2, w2, 0.0),
                         wall_mode=WALL_ONESIDED, sched_mode=SCHED_LINEAR, R0=150.0, R1=50.0,
-                        sched_steps=20000, seed=3, steps=20000, init="ball", tuned_cells_per_cut=[1, 2, 2],
-                        tuned_neighbour_list=(0.5, 256))
+                        sched_steps=20000, seed=3, steps=20000, init="ball")
     if name == "C4":
         s = [1.0]
         n = 250000
@@ -110,16 +101,14 @@ def _spec(name: str) -> Workload:
                         kT=0.5, dt=0.001, cut_factor=2.5, coulomb_k=0.0, g=0.0,
                         omega2=(0.0, 0.0, 0.0), wall_mode=WALL_ONESIDED,
                         sched_mode=SCHED_CONST, R0=R, R1=R, sched_steps=0,
-                        seed=4, steps=5000, init="fcc", tuned_cells_per_cut=[3],
-                        tuned_neighbour_list=(0.2, 160))
+                        seed=4, steps=5000, init="fcc")
     if name == "C5":
         s = [1.0, 1.2]
         return Workload("C5", 1048576, s, [1.0, 1.0], [0.5, -0.5], _mass(s), [100.0] * 2,
                         [1.0] * 2, [0.5, 0.5], kT=1.0, dt=0.002, cut_factor=4.0,
                         coulomb_k=0.7, g=0.0, omega2=(0.0, 0.0, 0.0),
                         wall_mode=WALL_ONESIDED, sched_mode=SCHED_LINEAR, R0=250.0, R1=120.0,
-                        sched_steps=10000, seed=5, steps=10000, init="ball", tuned_cells_per_cut=[1, 1],
-                        tuned_neighbour_list=(0.4, 128))
+                        sched_steps=10000, seed=5, steps=10000, init="ball")
     # ---- paper-shaped scenarios (Table 1) in reduced units; synthetic
     # stand-ins: the authors' parameter files are not available
     if name == "T8":
@@ -131,7 +120,7 @@ def _spec(name: str) -> Workload:
                         [0.2, 0.15, 0.15, 0.1, 0.1, 0.1, 0.1, 0.1], kT=1.0, dt=0.002, cut_factor=3.0,
                         coulomb_k=0.7, g=0.01, omega2=(2.5e-5, 2.5e-5, 0.0), wall_mode=WALL_ONESIDED,
                         sched_mode=SCHED_LINEAR, R0=45.0, R1=25.0, sched_steps=5000, seed=21,
-                        steps=5000, init="ball", tuned_cells_per_cut=[1] * 8)
+                        steps=5000, init="ball")
     if name == "P1":
         # row "1" (Fig. 2, 7): R0 = 20 um, r_NP = 0.5 um -> sigma = 1, R0 = 20; 10^4 neutral NPs,
         # LJ only, range 4 (r_A + r_B), no evaporation, random tumbling =
@@ -142,8 +131,7 @@ def _spec(name: str) -> Workload:
                         kT=1.0, dt=0.005, cut_factor=4.0, coulomb_k=0.0, g=0.0,
                         omega2=(w2, w2, w2), wall_mode=WALL_WINDOW,
                         sched_mode=SCHED_CONST, R0=20.0, R1=20.0, sched_steps=0,
-                        seed=11, steps=5000, init="ball", tuned_cells_per_cut=[2],
-                        tuned_neighbour_list=(0.3, 256))
+                        seed=11, steps=5000, init="ball")
     if name == "P8":
         # row "8" (Fig. 8, 9): R0 = 60 um, r_NP = 0.25 / 1.5 um (6 : 1) -> sigma = 1 / 6,
         # R0 = 120; 39 500 + 1 500 neutral NPs; eps = 0.23 [[0.155, 0.155], [0, 1.26]] is not a
@@ -157,8 +145,7 @@ def _spec(name: str) -> Workload:
                         [1.0] * 2, [39500.0 / 41000.0, 1500.0 / 41000.0], kT=1.0, dt=0.002,
                         cut_factor=4.0, coulomb_k=0.0, g=0.0, omega2=(w2, w2, 0.0),
                         wall_mode=WALL_ONESIDED, sched_mode=SCHED_R2LAW, R0=120.0, R1=48.0,
-                        sched_steps=20000, seed=18, steps=20000, init="ball", eps_matrix=eps,
-                        tuned_cells_per_cut=[1, 3], tuned_neighbour_list=(0.4, 512))
+                        sched_steps=20000, seed=18, steps=20000, init="ball", eps_matrix=eps)
     raise KeyError(name)
 
 

@@ -7,7 +7,7 @@ and positions <= 1e-5 (relative to |v| + sqrt(kT/m), resp. R); 100 steps
 import numpy as np
 import pytest
 
-from paper_2501_04456_b200 import workloads as W
+from paper_2501_04456_b200 import tuning, workloads as W
 
 pytestmark = pytest.mark.gpu
 
@@ -105,7 +105,7 @@ def test_forces_full_size(B, orc, name):
     w = workload(name, None)
     p = orc.params_from_workload(w)
     Fo, So, co, _ = orc.pair_forces(p, w.pos, w.type, "cells")
-    sim = B.Simulation.from_workload(w, cells_per_cut=w.tuned_cells_per_cut)
+    sim = B.Simulation.from_workload(w, cells_per_cut=tuning.cells_per_cut(w))
     sim.compute_forces()
     Fg, cg = sim.get_forces()
     assert np.array_equal(cg, co)
@@ -193,7 +193,7 @@ def test_hundred_steps(B, orc, name, n, cpc):
     droplet radius"), C3 -- the bench workload -- also at full size with its tuned grids."""
     w = workload(name, n)
     if cpc == "tuned":
-        cpc = w.tuned_cells_per_cut
+        cpc = tuning.cells_per_cut(w)
     p = orc.params_from_workload(w)
     xo, vo, bad = orc.step(p, w.pos, w.vel, w.type, step0=0, nsteps=100)
     sim = B.Simulation.from_workload(w, cells_per_cut=cpc)
@@ -214,7 +214,7 @@ def test_forces_at_the_benched_snapshots(B, orc):
     default kernel and with the shared-candidate-stream kernel."""
     w = workload("C3", None)
     p = orc.params_from_workload(w)
-    cpc = w.tuned_cells_per_cut
+    cpc = tuning.cells_per_cut(w)
     sim = B.Simulation.from_workload(w, cells_per_cut=cpc)
     tile = B.Simulation.from_workload(w, cells_per_cut=cpc, load_state=False,
                                       options={B.OPT_FORCE_KERNEL: B.FORCE_TILE, B.OPT_TILE_SUBSTREAMS: 8})
@@ -395,7 +395,7 @@ def test_full_size_trajectory_in_the_bench_configuration(B, orc):
     oracle, every NP compared by id."""
     w = workload("C3", None)
     p = orc.params_from_workload(w)
-    sim = B.Simulation.from_workload(w, cells_per_cut=w.tuned_cells_per_cut)
+    sim = B.Simulation.from_workload(w, cells_per_cut=tuning.cells_per_cut(w))
     x1o, v1o, bad = orc.step(p, w.pos, w.vel, w.type, step0=0, nsteps=1)
     assert bad == 0
     sim.step(1)
@@ -422,7 +422,7 @@ def test_paper_shaped_scenarios(B, orc, name):
     bit-exact, forces to 1e-5, 100 steps to 1e-3 R, with and without the neighbour list."""
     w = workload(name, None)
     p = orc.params_from_workload(w)
-    cpc = w.tuned_cells_per_cut
+    cpc = tuning.cells_per_cut(w)
     g = orc.grid_spec(p, cpc)
     key, ks, perm, off = orc.cell_structures(g, w.pos, w.type)
     Fo, So, co, _ = orc.pair_forces(p, w.pos, w.type, "cells")
@@ -440,7 +440,7 @@ def test_paper_shaped_scenarios(B, orc, name):
     x, v, _, R, st = sim.get_state()
     assert st == 100 and R == pytest.approx(orc.radius(p, 100), rel=1e-15)
     assert np.linalg.norm(x.astype(np.float64) - xo, axis=1).max() <= 1e-3 * R
-    lst = B.Simulation.from_workload(w, cells_per_cut=cpc, neighbour_list=w.tuned_neighbour_list)
+    lst = B.Simulation.from_workload(w, cells_per_cut=cpc, neighbour_list=tuning.neighbour_list(w))
     lst.step(100)
     xl, vl, _, _, _ = lst.get_state()
     assert np.linalg.norm(xl.astype(np.float64) - xo, axis=1).max() <= 1e-3 * R
@@ -513,7 +513,7 @@ def test_replica_set_equals_solo_runs(B, orc, batched):
     rs.synchronize()
     got = [rs.get_state(r) for r in range(5)]
     for r in range(5):
-        solo = B.Simulation.from_workload(rs.workloads[r], cells_per_cut=rs.workloads[r].tuned_cells_per_cut)
+        solo = B.Simulation.from_workload(rs.workloads[r], cells_per_cut=tuning.cells_per_cut(rs.workloads[r]))
         solo.step(40)
         ref = solo.get_state()
         for u, v in zip(got[r][:3], ref[:3]):

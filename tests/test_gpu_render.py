@@ -3,7 +3,7 @@ same splat: every pixel bit-exact."""
 import numpy as np
 import pytest
 
-from paper_2501_04456_b200 import workloads as W
+from paper_2501_04456_b200 import tuning, workloads as W
 
 pytestmark = pytest.mark.gpu
 
@@ -71,7 +71,7 @@ def test_surface_map_bit_exact(B, orc, name, n, cpc, steps, WH, min_marks):
     """lv_render_surface (Fig. 2 left panel) against the oracle's per-pixel brute force."""
     w = W.make_workload(name, n)
     ra = 0.5 * np.asarray(w.sigma)
-    sim = B.Simulation.from_workload(w, cells_per_cut=cpc if cpc is not None else w.tuned_cells_per_cut)
+    sim = B.Simulation.from_workload(w, cells_per_cut=cpc if cpc is not None else tuning.cells_per_cut(w))
     if steps:
         sim.step(steps)
     x, v, t, R, st = sim.get_state()
@@ -84,7 +84,7 @@ def test_surface_map_bit_exact(B, orc, name, n, cpc, steps, WH, min_marks):
     sim.synchronize()
     assert np.array_equal(dev.cpu().numpy().view(np.uint32), ref)
     # the map does not disturb the run
-    ref_sim = B.Simulation.from_workload(w, cells_per_cut=cpc if cpc is not None else w.tuned_cells_per_cut)
+    ref_sim = B.Simulation.from_workload(w, cells_per_cut=cpc if cpc is not None else tuning.cells_per_cut(w))
     ref_sim.step(steps + 20); sim.step(20)
     xa, va, _, _, _ = sim.get_state()
     xb, vb, _, _, _ = ref_sim.get_state()
