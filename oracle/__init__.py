@@ -51,7 +51,9 @@ _lib = None
 def lib():
     global _lib
     if _lib is None:
-        path = _build.build()
+        # LV_ORACLE_LIB: another build of the same source (the sanitizer target of
+        # tests/test_oracle_sanitize.py)
+        path = os.environ.get("LV_ORACLE_LIB") or _build.build()
         L = C.CDLL(path)
         dp = C.POINTER(C.c_double)
         fp = C.POINTER(C.c_float)

@@ -21,5 +21,15 @@ def build(force: bool = False) -> str:
     return LIB
 
 
+def build_sanitized(out_path: str) -> str:
+    """The same source with AddressSanitizer + UndefinedBehaviorSanitizer, for
+    tests/test_oracle_sanitize.py; loaded through LV_ORACLE_LIB under LD_PRELOAD=libasan."""
+    cmd = ["gcc", "-O1", "-g", "-std=c11", "-ffp-contract=off", "-fno-fast-math", "-fopenmp",
+           "-fsanitize=address,undefined", "-fno-sanitize-recover=undefined", "-fno-omit-frame-pointer",
+           "-fPIC", "-shared", "-Wall", "-Wextra", "-o", out_path, SRC, "-lm"]
+    subprocess.run(cmd, check=True, cwd=HERE)
+    return out_path
+
+
 if __name__ == "__main__":
     print(build(force=True))
