@@ -473,6 +473,11 @@ def run_lv(args):
         "ncu": ({"report": rec["report"], "duration_us": rec["duration_us"], "issue_active_pct": rec["issue_active_pct"],
                  "l1_data_pipe_pct": rec["l1_data_pipe_pct"], "lts_bytes": rec["lts_bytes"],
                  "source_hash": rec["source_hash"], "stale": rec["stale"]} if rec is not None else None),
+        # the same kernel against the HBM roofline: its measured DRAM traffic (the list is streamed
+        # once per launch) over the kernel time, of the measured copy bandwidth
+        "hbm": ({"achieved": rec["dram_bytes"] / (force_ms * 1e-3) * 1e-9, "peak": pk["hbm_gbs"], "unit": "GB/s",
+                 "frac": rec["dram_bytes"] / (force_ms * 1e-3) * 1e-9 / pk["hbm_gbs"],
+                 "peak_source": pk["source"]} if usable else None),
         "kernel_ms": force_ms,
         "share_of_step": stages["pair_force"] / tot_ms,          # against the graph-replayed (headline) step
         "share_of_stage_pass": stages["pair_force"] / stage_tot_ms,   # that pass carries event overhead
