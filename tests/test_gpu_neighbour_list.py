@@ -208,3 +208,32 @@ def test_needs_the_counting_sort(B):
     w = W.make_workload("C1")
     with pytest.raises(B.LvError):
         B.Simulation.from_workload(w, options={B.OPT_SORT: B.SORT_RADIX}, neighbour_list=(0.3, 64))
+
+
+@pytest.mark.parametrize("lanes", [1, 2, 4, 8, 16, 32])
+def test_lanes_per_np_do_not_change_results(B, lanes):
+    """LV_OPT_LIST_LANES: 1 .. 32 lanes sharing an NP's list give bit-identical neighbour counts
+    and forces equal to rounding (different summation order), against a cell evaluation of the
+    same state; 60 further steps stay close to the automatic choice."""
+    w = W.make_workload("C3", 20000)
+    cpc = [1, 2, 2]
+    lst = B.Simulation.from_workload(w, cells_per_cut=cpc, neighbour_list=(0.5, -1),
+                                     options={B.OPT_LIST_LANES: lanes})
+    cel = B.Simulation.from_workload(w, cells_per_cut=cpc, neighbour_list=None)
+    lst.step(5)
+    x, v, t, R, st = lst.get_state()
+    cel.set_state(x, v, t, step=st)
+    cel.compute_forces()
+    Fc, cc = cel.get_forces()
+    lst.step(1)
+    Fl, cl = lst.get_forces()
+    assert lst.list_stats()["lanes_per_np"] in (4, 8) and lst.rebuild_count() >= 1
+    assert np.array_equal(cl, cc) and cc.sum() > 0
+    S = np.abs(Fc).sum(axis=1) + np.abs(Fc).max()
+    assert np.max(np.abs(Fl - Fc).max(axis=1) / S) <= 1e-4
+    auto = B.Simulation.from_workload(w, cells_per_cut=cpc, neighbour_list=(0.5, -1))
+    auto.step(66); lst.step(60)
+    xa, xl = auto.get_state()[0], lst.get_state()[0]
+    assert np.abs(xa - xl).max() <= 1e-3
+    for s in (lst, cel, auto):
+        s.close()
