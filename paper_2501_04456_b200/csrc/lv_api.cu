@@ -338,11 +338,11 @@ void free_timing(lv_sim *s)
 // List step as a graph with an IF node: [condition kernel] -> IF(rebuild flag){ rebuild chain:
 // stages 0..2 } -> list force, cell force (guarded) -> update.  The body is captured on a
 // helper stream into the conditional node's body graph.
-int capture_list_step(lv_sim *s, cudaGraph_t g, cudaGraph_t *body_out)
+// `s->stream` is capturing into graph `g` (as the origin or joined to it): append one list step.
+int enqueue_list_step_if(lv_sim *s, cudaGraph_t g, cudaGraph_t *body_out)
 {
     cudaGraphConditionalHandle h;
     LV_CUDA(s, cudaGraphConditionalHandleCreate(&h, g, 0, 0));
-    LV_CUDA(s, cudaStreamBeginCaptureToGraph(s->stream, g, nullptr, nullptr, 0, cudaStreamCaptureModeRelaxed));
     int rc = LV_OK;
     cudaError_t e = lvk_list_cond((unsigned long long)h, s->bufs, s->stream);
     cudaStream_t helper = nullptr;
@@ -363,7 +363,7 @@ int capture_list_step(lv_sim *s, cudaGraph_t g, cudaGraph_t *body_out)
         if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&helper, cudaStreamNonBlocking);
         if (e == cudaSuccess) {
             cudaGraph_t body = np.conditional.phGraph_out[0];
-            *body_out = body;
+            if (body_out) *body_out = body;
             e = cudaStreamBeginCaptureToGraph(helper, body, nullptr, nullptr, 0, cudaStreamCaptureModeRelaxed);
             if (e == cudaSuccess) {
                 cudaStream_t keep = s->stream;
@@ -377,12 +377,19 @@ int capture_list_step(lv_sim *s, cudaGraph_t g, cudaGraph_t *body_out)
         }
     }
     for (int k = 3; k < LV_N_STAGES && rc == LV_OK && e == cudaSuccess; ++k) rc = enqueue_stage(s, k, true);
-    cudaGraph_t gout = nullptr;
-    cudaError_t e3 = cudaStreamEndCapture(s->stream, &gout);
     if (helper) cudaStreamDestroy(helper);
-
     if (rc != LV_OK) return rc;
     if (e != cudaSuccess) return cuda_fail(s, e, "capture of the list step");
+    return LV_OK;
+}
+
+int capture_list_step(lv_sim *s, cudaGraph_t g, cudaGraph_t *body_out)
+{
+    LV_CUDA(s, cudaStreamBeginCaptureToGraph(s->stream, g, nullptr, nullptr, 0, cudaStreamCaptureModeRelaxed));
+    int rc = enqueue_list_step_if(s, g, body_out);
+    cudaGraph_t gout = nullptr;
+    cudaError_t e3 = cudaStreamEndCapture(s->stream, &gout);
+    if (rc != LV_OK) return rc;
     if (e3 != cudaSuccess) return cuda_fail(s, e3, "cudaStreamEndCapture");
     return LV_OK;
 }
@@ -1221,15 +1228,22 @@ namespace {
 int capture_batch(lv_batch *b, int steps, cudaGraph_t *g, cudaGraphExec_t *x)
 {
     lv_sim *s0 = b->sims[0];
-    LV_CUDA(s0, cudaStreamBeginCapture(s0->stream, cudaStreamCaptureModeRelaxed));
+    cudaGraph_t gg = nullptr;
+    LV_CUDA(s0, cudaGraphCreate(&gg, 0));
+    cudaError_t e = cudaStreamBeginCaptureToGraph(s0->stream, gg, nullptr, nullptr, 0, cudaStreamCaptureModeRelaxed);
+    if (e != cudaSuccess) { cudaGraphDestroy(gg); return cuda_fail(s0, e, "cudaStreamBeginCaptureToGraph"); }
     int rc = LV_OK;
-    cudaError_t e = cudaEventRecord(b->ev[0], s0->stream);
+    e = cudaEventRecord(b->ev[0], s0->stream);
     for (int r = 1; r < b->n && e == cudaSuccess; ++r) e = cudaStreamWaitEvent(b->sims[r]->stream, b->ev[0], 0);
     for (int r = 0; r < b->n && e == cudaSuccess && rc == LV_OK; ++r) {
         lv_sim *s = b->sims[r];
         for (int k = 0; k < steps && rc == LV_OK; ++k) {
-            s->hashed = s->sort_mode == LV_SORT_COUNTING && s->list_cap == 0;     // steady-state step
-            rc = enqueue_step(s);
+            if (s->list_cap != 0) {          // list step: its own IF node around the rebuild chain
+                rc = enqueue_list_step_if(s, gg, nullptr);
+            } else {
+                s->hashed = s->sort_mode == LV_SORT_COUNTING;     // steady-state step
+                rc = enqueue_step(s);
+            }
         }
         s->hashed = false;
         if (r > 0 && rc == LV_OK) {
@@ -1237,15 +1251,16 @@ int capture_batch(lv_batch *b, int steps, cudaGraph_t *g, cudaGraphExec_t *x)
             if (e == cudaSuccess) e = cudaStreamWaitEvent(s0->stream, b->ev[r], 0);
         }
     }
-    cudaGraph_t gg = nullptr;
-    cudaError_t e2 = cudaStreamEndCapture(s0->stream, &gg);
+    cudaGraph_t gout = nullptr;
+    cudaError_t e2 = cudaStreamEndCapture(s0->stream, &gout);
+    (void)cudaGetLastError();
     if (rc == LV_OK && e != cudaSuccess) rc = cuda_fail(s0, e, "lv_batch capture");
     if (rc == LV_OK && e2 != cudaSuccess) rc = cuda_fail(s0, e2, "cudaStreamEndCapture");
     if (rc == LV_OK) {
         e2 = cudaGraphInstantiate(x, gg, 0);
         if (e2 != cudaSuccess) rc = cuda_fail(s0, e2, "cudaGraphInstantiate");
     }
-    if (rc != LV_OK) { if (gg) cudaGraphDestroy(gg); return rc; }
+    if (rc != LV_OK) { cudaGraphDestroy(gg); return rc; }
     *g = gg;
     return LV_OK;
 }

@@ -890,6 +890,9 @@ k_pair_force_s(const __grid_constant__ LvDev P, const float4 *__restrict__ pos,
 constexpr int kRThreads = 128;
 constexpr int kRPerWarp = 8;        // NPs per warp: small work items, balanced by the block scheduler
 
+#ifndef LV_ROWS_MINB
+#define LV_ROWS_MINB 10             // 48 registers: 40 resident warps (6 and 8 candidates per round, at 79 / 95 registers, were slower)
+#endif
 template <bool kCharged, int S>
 __device__ __forceinline__ void rows_body(const LvDev &P, const float4 *__restrict__ pos,
                                           const uint32_t *__restrict__ list,
@@ -897,6 +900,7 @@ __device__ __forceinline__ void rows_body(const LvDev &P, const float4 *__restri
                                           const uint32_t *__restrict__ list_len,
                                           float4 *__restrict__ force, const LvPair *s_pair)
 {
+    constexpr int U = 4;                                // candidates per lane and round
     constexpr int T = 32 / S;
     constexpr int G = T > kRPerWarp ? T : kRPerWarp;    // NPs per warp
     const int lane = threadIdx.x & 31;
@@ -918,27 +922,27 @@ __device__ __forceinline__ void rows_body(const LvDev &P, const float4 *__restri
         const uint32_t *lp = list + b0 + ls;
         float fx = 0.f, fy = 0.f, fz = 0.f;
         int cnt = 0;
+        int tcur = -1;                          // type whose pair constants are in prc
+        LvPair prc = {0.f, 0.f, 0.f, 0.f};
         // Gather u of a round takes the S CONSECUTIVE entries u S .. u S + S - 1 of every NP of
         // the group (ascending slots: few cache lines per request).  Software pipeline: the
         // indices of the next round are loading while this one is evaluated.
-        uint32_t jn[4];
+        uint32_t jn[U];
 #pragma unroll
-        for (int u = 0; u < 4; ++u) jn[u] = (uint32_t)(u * S + ls) < len ? __ldg(lp + u * S) : self;
-        for (uint32_t k0 = 0; k0 < maxlen; k0 += 4u * S) {
-            uint32_t jj[4];
+        for (int u = 0; u < U; ++u) jn[u] = (uint32_t)(u * S + ls) < len ? __ldg(lp + u * S) : self;
+        for (uint32_t k0 = 0; k0 < maxlen; k0 += (uint32_t)(U * S)) {
+            uint32_t jj[U];
 #pragma unroll
-            for (int u = 0; u < 4; ++u) jj[u] = jn[u];
+            for (int u = 0; u < U; ++u) jj[u] = jn[u];
 #pragma unroll
-            for (int u = 0; u < 4; ++u) {
-                const uint32_t kn = k0 + (uint32_t)((4 + u) * S + ls);
-                jn[u] = kn < len ? __ldg(lp + (k0 + (uint32_t)((4 + u) * S))) : self;
+            for (int u = 0; u < U; ++u) {
+                const uint32_t kn = k0 + (uint32_t)((U + u) * S + ls);
+                jn[u] = kn < len ? __ldg(lp + (k0 + (uint32_t)((U + u) * S))) : self;
             }
-            float4 pj[4];
+            float4 pj[U];
 #pragma unroll
-            for (int u = 0; u < 4; ++u) pj[u] = __ldg(pos + jj[u]);
-#pragma unroll
-            for (int u = 0; u < 4; ++u) {
-                const LvPair pr = pair_a[__float_as_int(pj[u].w)];
+            for (int u = 0; u < U; ++u) pj[u] = __ldg(pos + jj[u]);
+            auto eval = [&](const LvPair &pr, int u) {
                 const float dx = __fsub_rn(pi.x, pj[u].x);
                 const float dy = __fsub_rn(pi.y, pj[u].y);
                 const float dz = __fsub_rn(pi.z, pj[u].z);
@@ -955,6 +959,23 @@ __device__ __forceinline__ void rows_body(const LvDev &P, const float4 *__restri
                 fy = fmaf(f, dy, fy);
                 fz = fmaf(f, dz, fz);
                 cnt += in ? 1 : 0;
+            };
+            // A list holds its candidates grid by grid, i.e. TYPE BY TYPE: the pair constants of
+            // the last candidate stay in registers and a round whose four candidates are of that
+            // type reads none from shared memory (16 bytes per lane and candidate less through
+            // the load/store unit, which bounds this kernel)
+            bool same = true;
+#pragma unroll
+            for (int u = 0; u < U; ++u) same = same && __float_as_int(pj[u].w) == tcur;
+            if (same) {
+#pragma unroll
+                for (int u = 0; u < U; ++u) eval(prc, u);
+            } else {
+#pragma unroll
+                for (int u = 0; u < U - 1; ++u) eval(pair_a[__float_as_int(pj[u].w)], u);
+                tcur = __float_as_int(pj[U - 1].w);
+                prc = pair_a[tcur];
+                eval(prc, U - 1);
             }
         }
 #pragma unroll
@@ -969,7 +990,7 @@ __device__ __forceinline__ void rows_body(const LvDev &P, const float4 *__restri
 }
 
 template <bool kCharged>
-__global__ void __launch_bounds__(kRThreads)
+__global__ void __launch_bounds__(kRThreads, LV_ROWS_MINB)
 k_pair_force_rows(const __grid_constant__ LvDev P, const float4 *__restrict__ posA,
                   const float4 *__restrict__ posB, const uint32_t *__restrict__ list,
                   const uint32_t *__restrict__ list_start, const uint32_t *__restrict__ list_len,

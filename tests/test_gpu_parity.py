@@ -529,6 +529,34 @@ def test_replica_set_equals_solo_runs(B, orc, batched):
     rs.close()
 
 
+def test_batched_replicas_with_neighbour_lists_equal_solo_runs(B):
+    """lv_batch with the skin list on: every replica's steps sit in the one graph with their own
+    IF node around the rebuild chain (replicas rebuild at different steps); each replica is
+    bit-identical to the same workload stepped alone with the same list setting, and its list
+    was rebuilt as often."""
+    from paper_2501_04456_b200 import replicas
+    mk = lambda seed: W.make_workload("C2", 3001, seed=seed)
+    nl = (0.4, 256)
+    rs = replicas.ReplicaSet(mk, 4, base_seed=5, batched=True, steps_per_launch=5, neighbour_list=nl)
+    rs.step(3)
+    rs.step(64)                      # chunks of 5 and single steps
+    rs.synchronize()
+    for r in range(4):
+        got = rs.get_state(r)
+        solo = B.Simulation.from_workload(rs.workloads[r], cells_per_cut=tuning.cells_per_cut(rs.workloads[r]),
+                                          neighbour_list=nl)
+        solo.step(67)
+        ref = solo.get_state()
+        for u, v in zip(got[:3], ref[:3]):
+            assert np.array_equal(u, v)
+        assert got[3:] == ref[3:]
+        assert rs.sims[r].status() == 0
+        ls, lr = rs.sims[r].list_stats(), solo.list_stats()
+        assert ls["rebuilds"] == lr["rebuilds"] >= 2 and ls["fallback_steps"] == lr["fallback_steps"]
+        solo.close()
+    rs.close()
+
+
 def test_restart_continues_within_tolerance(B):
     """Stop, save, restart (PAPER.md:84): same noise (keyed on id and step);
     only the summation order changes, so the continuation agrees to rounding."""
