@@ -239,10 +239,13 @@ int enqueue_stage(lv_sim *s, int stage, bool list_step = false)
             LV_CUDA(s, lvk_place(s->dev, s->bufs, true, s->stream));
             LV_CUDA(s, lvk_rank_gather(s->dev, s->bufs, false, true, s->stream));
             LV_CUDA(s, lvk_list_build(s->dev, s->bufs, s->stream));
+            // the cell kernel of a step whose list does not fit (or is deferred): such a step
+            // always rebuilds the cells, so the kernel sits with the rebuild chain -- inside the
+            // IF node of the step graph -- and an ordinary step does not launch it at all
+            LV_CUDA(s, lvk_pair_force_fallback(s->dev, s->bufs, s->stream));
             break;
         case 3:
             LV_CUDA(s, lvk_pair_force_list(s->dev, s->bufs, s->stream));
-            LV_CUDA(s, lvk_pair_force_fallback(s->dev, s->bufs, s->stream));    // only while the list does not fit
             break;
         default: LV_CUDA(s, lvk_update_list(s->dev, s->bufs, s->stream)); break;
         }

@@ -881,7 +881,7 @@ k_pair_force_s(const __grid_constant__ LvDev P, const float4 *__restrict__ pos,
 // candidates that mostly sit in the same or neighbouring cache lines (the lane-per-NP tiles
 // of round 1 gathered from ~25 different lines per request); the S partial sums are added by
 // xor shuffles in a fixed order.  S is chosen on the device at every rebuild from the mean
-// list length (LvDevState::list_lanes: 4 below 64 entries, else 8; LV_OPT_LIST_LANES forces it).
+// list length (LvDevState::list_lanes: 4 below 256 entries, else 8; LV_OPT_LIST_LANES forces it).
 // The positions are those of the list's slot order: posB on the step that rebuilt, else posA
 // (k_update keeps that order until the next rebuild).
 #ifndef LV_LIST_MARGIN
@@ -1053,7 +1053,7 @@ __global__ void k_list_check(int n, uint32_t pool, bool exact, LvDevState *st)
     // lanes per NP from the mean TRUE length: the count itself (exact build) or the previous
     // list's (one-walk build: its reserve is ~1.5 x the length for short lists)
     const unsigned long long mean = (exact ? total : st->list_true) / (unsigned long long)(n > 0 ? n : 1);
-    st->list_lanes = mean < 64ull ? 4u : 8u;          // measured on C3
+    st->list_lanes = mean < 256ull ? 4u : 8u;         // measured on C3 and C4
     st->list_true = 0ull;                             // the fill that follows sums the new one
     if (!fits) atomicOr(&st->status, LV_ST_LIST_OVERFLOW);
 }
