@@ -137,8 +137,9 @@ Layout layout_of(const lv_sim *s)
     const size_t n = (size_t)(s->n > 0 ? s->n : 1);
     size_t o = 0;
     auto take = [&](size_t bytes) { size_t at = o; o = align_up(o + bytes); return at; };
-    L.posA = take(16 * n); L.velA = take(16 * n);
-    L.posB = take(16 * n); L.velB = take(16 * n);
+    // positions: one slot more, a dummy far outside every cut-off (the padding of the skin lists points at it)
+    L.posA = take(16 * (n + 1)); L.velA = take(16 * n);
+    L.posB = take(16 * (n + 1)); L.velB = take(16 * n);
     L.force = take(16 * n);
     L.key_in = take(4 * n); L.key_out = take(4 * n);
     L.val_in = take(4 * n); L.val_out = take(4 * n);

@@ -113,7 +113,7 @@ struct LvBufs {
     // outside every cut-off.  Written by the gather only when that kernel is selected.
     float *posP;
     // skin neighbour list: the NP at sorted slot i owns list[list_start[i] .. list_start[i + 1]),
-    // its neighbours' slots in walk order, padded to a multiple of 4 entries with its own slot;
+    // its neighbours' slots in walk order, padded to a multiple of 4 entries with the dummy slot n (posA[n] = posB[n]: far outside every cut-off);
     // list_cnt = padded lengths (input of the scan, zero between builds), list_start = their
     // exclusive scan; pos_ref = positions at the last build.
     uint32_t *list;

@@ -849,18 +849,19 @@ k_pair_force_s(const __grid_constant__ LvDev P, const float4 *__restrict__ pos,
     }
     if (kList) {
         // lengths are padded to a multiple of 4 entries (16-byte stores and starts); the padding
-        // holds the NP's own slot, which the force kernel rejects by j != i
+        // points at the dummy slot n, far outside every cut-off
         if (kCount) {
             const uint32_t padded = live ? ((uint32_t)cnt + 3u) & ~3u : 0u;
             if (live) LA.cnt[i] = padded;
             const uint32_t wsum = __reduce_add_sync(kFull, padded);
             if ((gtid & 31) == 0 && wsum) atomicAdd(&st->list_total, (unsigned long long)wsum);
         } else {
-            const int q = cnt & 3;              // the last, partial group: padded with the NP's own slot
+            const int q = cnt & 3;              // the last, partial group: padded with the dummy slot
             if (live && q != 0 && cnt < cap) {
-                ebuf.y = q > 1 ? ebuf.y : self;
-                ebuf.z = q > 2 ? ebuf.z : self;
-                ebuf.w = self;
+                const uint32_t dummy = (uint32_t)P.n;
+                ebuf.y = q > 1 ? ebuf.y : dummy;
+                ebuf.z = q > 2 ? ebuf.z : dummy;
+                ebuf.w = dummy;
                 col[cnt >> 2] = ebuf;
             }
             const uint32_t tlen = live ? ((uint32_t)cnt + 3u) & ~3u : 0u;
@@ -891,7 +892,7 @@ constexpr int kRThreads = 128;
 constexpr int kRPerWarp = 8;        // NPs per warp: small work items, balanced by the block scheduler
 
 #ifndef LV_ROWS_MINB
-#define LV_ROWS_MINB 10             // 48 registers: 40 resident warps (6 and 8 candidates per round, at 79 / 95 registers, were slower)
+#define LV_ROWS_MINB 9              // 56 registers, 36 resident warps (measured against 48 and 72; 6 and 8 candidates per round, at 79 / 95 registers, were slower)
 #endif
 template <bool kCharged, int S>
 __device__ __forceinline__ void rows_body(const LvDev &P, const float4 *__restrict__ pos,
@@ -913,8 +914,8 @@ __device__ __forceinline__ void rows_body(const LvDev &P, const float4 *__restri
     for (int g0 = 0; g0 < G; g0 += T) {
         const int i = wbase + g0 + lt;
         const bool live = i >= 0;
-        const uint32_t self = live ? (uint32_t)i : 0u;
-        const float4 pi = pos[self];
+        const uint32_t dummy = (uint32_t)P.n;       // pos[n]: far outside every cut-off
+        const float4 pi = pos[live ? (uint32_t)i : dummy];
         const LvPair *pair_a = s_pair + (live ? __float_as_int(pi.w) : 0) * LV_MAX_TYPES;
         const uint32_t b0 = live ? __ldg(list_start + i) : 0u;
         const uint32_t len = live ? __ldg(list_len + i) : 0u;                // a multiple of 4
@@ -929,7 +930,7 @@ __device__ __forceinline__ void rows_body(const LvDev &P, const float4 *__restri
         // indices of the next round are loading while this one is evaluated.
         uint32_t jn[U];
 #pragma unroll
-        for (int u = 0; u < U; ++u) jn[u] = (uint32_t)(u * S + ls) < len ? __ldg(lp + u * S) : self;
+        for (int u = 0; u < U; ++u) jn[u] = (uint32_t)(u * S + ls) < len ? __ldg(lp + u * S) : dummy;
         for (uint32_t k0 = 0; k0 < maxlen; k0 += (uint32_t)(U * S)) {
             uint32_t jj[U];
 #pragma unroll
@@ -937,7 +938,7 @@ __device__ __forceinline__ void rows_body(const LvDev &P, const float4 *__restri
 #pragma unroll
             for (int u = 0; u < U; ++u) {
                 const uint32_t kn = k0 + (uint32_t)((U + u) * S + ls);
-                jn[u] = kn < len ? __ldg(lp + (k0 + (uint32_t)((U + u) * S))) : self;
+                jn[u] = kn < len ? __ldg(lp + (k0 + (uint32_t)((U + u) * S))) : dummy;
             }
             float4 pj[U];
 #pragma unroll
@@ -947,7 +948,7 @@ __device__ __forceinline__ void rows_body(const LvDev &P, const float4 *__restri
                 const float dy = __fsub_rn(pi.y, pj[u].y);
                 const float dz = __fsub_rn(pi.z, pj[u].z);
                 const float r2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
-                const bool in = r2 < pr.rc2 && jj[u] != self;            // fp32 contract #2
+                const bool in = r2 < pr.rc2;        // fp32 contract #2 (a list never holds its own NP)
                 const float rinv = rsqrt_approx(r2);
                 const float ir2 = rinv * rinv;
                 const float ir6 = ir2 * ir2 * ir2;
@@ -961,21 +962,34 @@ __device__ __forceinline__ void rows_body(const LvDev &P, const float4 *__restri
                 cnt += in ? 1 : 0;
             };
             // A list holds its candidates grid by grid, i.e. TYPE BY TYPE: the pair constants of
-            // the last candidate stay in registers and a round whose four candidates are of that
-            // type reads none from shared memory (16 bytes per lane and candidate less through
-            // the load/store unit, which bounds this kernel)
-            bool same = true;
+            // the last candidate stay in registers and shared memory is read only when the type
+            // changes (16 bytes per lane and candidate less through the load/store unit)
+            if constexpr (S >= 8) {
+                // long lists: one test per round, the four evaluations independent of one another
+                bool same = true;
 #pragma unroll
-            for (int u = 0; u < U; ++u) same = same && __float_as_int(pj[u].w) == tcur;
-            if (same) {
+                for (int u = 0; u < U; ++u) same = same && __float_as_int(pj[u].w) == tcur;
+                if (same) {
 #pragma unroll
-                for (int u = 0; u < U; ++u) eval(prc, u);
+                    for (int u = 0; u < U; ++u) eval(prc, u);
+                } else {
+#pragma unroll
+                    for (int u = 0; u < U - 1; ++u) eval(pair_a[__float_as_int(pj[u].w)], u);
+                    tcur = __float_as_int(pj[U - 1].w);
+                    prc = pair_a[tcur];
+                    eval(prc, U - 1);
+                }
             } else {
+                // short lists (a type change every few candidates): a predicated reload per candidate
 #pragma unroll
-                for (int u = 0; u < U - 1; ++u) eval(pair_a[__float_as_int(pj[u].w)], u);
-                tcur = __float_as_int(pj[U - 1].w);
-                prc = pair_a[tcur];
-                eval(prc, U - 1);
+                for (int u = 0; u < U; ++u) {
+                    const int t = __float_as_int(pj[u].w);
+                    if (t != tcur) {
+                        prc = pair_a[t];
+                        tcur = t;
+                    }
+                    eval(prc, u);
+                }
             }
         }
 #pragma unroll
@@ -1219,11 +1233,13 @@ k_update(const __grid_constant__ LvDev P, const float4 *__restrict__ posB_,
 // ------------------------------------------------- state in / out (by id)
 __global__ void __launch_bounds__(kThreads)
 k_pack_state(int n, int n_types, const float *__restrict__ pos, const float *__restrict__ vel,
-             const int32_t *__restrict__ type, float4 *__restrict__ posA,
+             const int32_t *__restrict__ type, float4 *__restrict__ posA, float4 *__restrict__ posB,
              float4 *__restrict__ velA, LvDevState *st, long long step)
 {
     int i = blockIdx.x * kThreads + threadIdx.x;
     if (i == 0) {
+        // the dummy slot behind the last NP (no kernel writes it again)
+        posA[n] = posB[n] = make_float4(1.0e18f, 1.0e18f, 1.0e18f, __int_as_float(0));
         st->step = step; st->ticket = 0u;       // status: cleared by lvk_pack_state before the launch
         st->rebuild[step & 1] = 1u;            // skin list: the first step builds it
         st->rebuild[(step + 1) & 1] = 0u;
@@ -1880,7 +1896,7 @@ cudaError_t lvk_pack_state(const LvDev &P, const LvBufs &B, const float *pos, co
     // cleared ahead of the kernel: its threads raise LV_ST_BAD_TYPE with atomicOr
     cudaError_t e = cudaMemsetAsync(&B.st->status, 0, sizeof(B.st->status), st);
     if (e != cudaSuccess) return e;
-    k_pack_state<<<blocks_for(P.n), kThreads, 0, st>>>(P.n, P.n_types, pos, vel, type, B.posA, B.velA, B.st, step);
+    k_pack_state<<<blocks_for(P.n), kThreads, 0, st>>>(P.n, P.n_types, pos, vel, type, B.posA, B.posB, B.velA, B.st, step);
     return cudaGetLastError();
 }
 
