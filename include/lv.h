@@ -185,15 +185,15 @@ int lv_set_option(lv_sim *s, int option, int value);
  * contract #2, so the neighbour counts stay bit-identical and the forces agree to rounding),
  * and rebuilds cells + list on the device -- no host round trip -- at the first step after any
  * NP has moved farther than skin/2 from where it was at the build.
- *   skin      length units; <= 0: automatic, a tenth of the smallest cut-off (needs lv_set_types
+ *   skin      length units; <= 0: automatic, 0.16 of the smallest cut-off (needs lv_set_types
  *             first).
  *   capacity  > 0: the list pool holds capacity entries per NP ON AVERAGE (4 * capacity bytes per
- *             NP of workspace; a crowded NP may use more than its share); -1: automatic, 1024
+ *             NP of workspace; a crowded NP may use more than its share); -1: automatic, 2048
  *             entries per NP but at most 2 GiB, and no list at all below 16 384 NPs (such a
  *             step is bound by launch latency, not by the force kernel); 0 (default): the variant is off and every step
  *             rebuilds the cells, as the paper does.
  * The list is built in two passes (count the lengths, scan them, fill): every NP owns one
- * contiguous run of the pool, and 8, 16 or 32 lanes share an NP in the force kernel (chosen on
+ * contiguous run of the pool, and 4 or 8 lanes share an NP in the force kernel (chosen on
  * the device from the mean length).  If a rebuild would need more than the pool, nothing is lost: the
  * warning bit LV_ST_LIST_OVERFLOW is raised and the steps run on the cell kernel (rebuilding the
  * cells every step) until a later count -- taken every 64th step -- fits again.  The choice

@@ -120,12 +120,12 @@ struct Layout {
 };
 
 // Pool of the skin list in entries: list_cap per NP on average (a crowded NP may use more than
-// its share); automatic: 1024 entries per NP, at most 2 GiB.
+// its share); automatic: 2048 entries per NP, at most 2 GiB.
 size_t list_pool_of(const lv_sim *s)
 {
     if (s->list_cap == 0) return 0;
     const size_t n = (size_t)(s->n > 0 ? s->n : 1);
-    size_t entries = s->list_cap > 0 ? n * (size_t)s->list_cap : n * 1024;
+    size_t entries = s->list_cap > 0 ? n * (size_t)s->list_cap : n * 2048;
     if (s->list_cap < 0 && entries > ((size_t)1 << 29)) entries = (size_t)1 << 29;
     entries += 64;
     return entries > 0xfffffff0ull ? 0xfffffff0ull : entries;
@@ -589,12 +589,14 @@ int lv_set_neighbour_list(lv_sim *s, double skin, int capacity)
 {
     if (!s || !std::isfinite(skin) || capacity < -1 || capacity > (1 << 16)) return LV_E_ARG;
     if (s->bound) return LV_E_ORDER;
-    if (capacity != 0 && !(skin > 0.0)) {       // automatic skin: a tenth of the smallest cut-off
+    // automatic skin: 0.16 of the smallest cut-off (measured on C2 .. C5: a rebuild every ~25 steps
+    // instead of ~16 at a tenth pays for the ~8 % longer lists, in the dilute and in the dense states)
+    if (capacity != 0 && !(skin > 0.0)) {
         if (!s->types_set) return LV_E_ORDER;
         double rmin = s->rcut[0];
         for (int a = 0; a < s->n_types; ++a)
             for (int b = 0; b < s->n_types; ++b) rmin = std::fmin(rmin, s->rcut[a * LV_MAX_TYPES + b]);
-        skin = 0.1 * rmin;
+        skin = 0.16 * rmin;
     }
     s->skin = capacity != 0 ? skin : 0.0;
     s->list_cap = capacity;

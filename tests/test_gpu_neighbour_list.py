@@ -185,8 +185,8 @@ def test_list_follows_a_shrinking_droplet_into_the_fallback(B, orc):
 
 
 def test_automatic_skin_and_pool(B, orc):
-    """lv_set_neighbour_list(skin <= 0, capacity = -1): skin = a tenth of the smallest cut-off,
-    pool = 1024 entries per NP; first-step counts bit-exact, 100 steps within tolerance."""
+    """lv_set_neighbour_list(skin <= 0, capacity = -1): skin = 0.16 of the smallest cut-off,
+    pool = 2048 entries per NP; first-step counts bit-exact, 100 steps within tolerance."""
     w = W.make_workload("C3", 20000)
     p = orc.params_from_workload(w)
     Fo, So, co, _ = orc.pair_forces(p, w.pos, w.type, "cells")
@@ -199,7 +199,7 @@ def test_automatic_skin_and_pool(B, orc):
     xo, vo, bad = orc.step(p, w.pos, w.vel, w.type, step0=0, nsteps=100)
     assert bad == 0 and np.linalg.norm(x.astype(np.float64) - xo, axis=1).max() <= 1e-3 * R
     s = sim.list_stats()
-    assert s["pool_entries"] >= 1024 * w.n and s["fallback_steps"] == 0 and 1 <= s["rebuilds"] < 100
+    assert s["pool_entries"] >= 2048 * w.n and s["fallback_steps"] == 0 and 1 <= s["rebuilds"] < 100
     assert sim.status() == 0
     sim.close()
 
