@@ -964,23 +964,16 @@ __device__ __forceinline__ void rows_body(const LvDev &P, const float4 *__restri
             // A list holds its candidates grid by grid, i.e. TYPE BY TYPE: the pair constants of
             // the last candidate stay in registers and shared memory is read only when the type
             // changes (16 bytes per lane and candidate less through the load/store unit)
-            if constexpr (S >= 8) {
-                // long lists: one test per round, the four evaluations independent of one another
-                bool same = true;
+            bool same = true;
 #pragma unroll
-                for (int u = 0; u < U; ++u) same = same && __float_as_int(pj[u].w) == tcur;
-                if (same) {
+            for (int u = 0; u < U; ++u) same = same && __float_as_int(pj[u].w) == tcur;
+            if (S >= 8 && __all_sync(kFull, same)) {
+                // long lists: most rounds see one type in the whole warp -- one vote, and the four
+                // evaluations are independent of one another
 #pragma unroll
-                    for (int u = 0; u < U; ++u) eval(prc, u);
-                } else {
-#pragma unroll
-                    for (int u = 0; u < U - 1; ++u) eval(pair_a[__float_as_int(pj[u].w)], u);
-                    tcur = __float_as_int(pj[U - 1].w);
-                    prc = pair_a[tcur];
-                    eval(prc, U - 1);
-                }
+                for (int u = 0; u < U; ++u) eval(prc, u);
             } else {
-                // short lists (a type change every few candidates): a predicated reload per candidate
+                // a predicated reload per candidate (short lists change type every few candidates)
 #pragma unroll
                 for (int u = 0; u < U; ++u) {
                     const int t = __float_as_int(pj[u].w);
