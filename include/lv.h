@@ -47,7 +47,7 @@ extern "C" {
 #define LV_E_CUDA       -4   /* a CUDA runtime call failed; see lv_last_cuda_error */
 #define LV_E_NONFINITE  -5   /* sticky: a non-finite position or velocity appeared (R6) */
 #define LV_E_NOMEM      -6   /* host allocation failed */
-#define LV_E_CAPACITY   -7   /* reserved (was: skin list overflow; now a warning, LV_ST_LIST_OVERFLOW) */
+#define LV_E_CAPACITY   -7   /* a size beyond a fixed maximum of the library (lv_observe_rdf_noalloc) */
 
 /* droplet schedule modes: step (iii); radius-square law PAPER.md:58 */
 #define LV_SCHED_CONST   0
@@ -259,6 +259,21 @@ int lv_get_forces(lv_sim *s, float *force_xyz, int32_t *neigh_count, int on_devi
  * the droplet volume at the current step; no boundary correction, as printed
  * (PAPER.md:139).  Rebuilds the cell structures of the current state and walks them. */
 int lv_observe_rdf(lv_sim *s, double dr, int n_bins, uint64_t *hist, double *g);
+
+/* lv_observe_rdf_noalloc: the same result as lv_observe_rdf (Eq. 6; same
+ * kernel, same fp32 contract #4, hist bit-identical) for callers that cannot provide scratch or
+ * call an allocator: the histogram scratch of the pair walk is a file-scope device array of
+ * the library, LV_NOALLOC_MAX_BINS * 8 bytes = 32 KiB, held by every GPU that loads the library
+ * until the process exits (its device address is taken once per device, on the device that is
+ * current at the call -- the caller keeps the handle's device current, as for every call).
+ * The call makes no cudaMalloc / cudaFree and no host allocation.  n_bins > LV_NOALLOC_MAX_BINS:
+ * LV_E_CAPACITY and a line on stderr, nothing launched.  ALL calls of a process share the one
+ * array per GPU; it keeps the previous call's counts and is cleared on the handle's stream
+ * before the walk.  Two calls that overlap on the GPU (two handles on different streams of one
+ * device) RACE on it: serialise them.  hist, g: host memory, written; either may be NULL.
+ * Synchronises the stream and leaves the state unchanged. */
+#define LV_NOALLOC_MAX_BINS 4096
+int lv_observe_rdf_noalloc(lv_sim *s, double dr, int n_bins, uint64_t *hist, double *g);
 
 /* lv_observe_radial: hist[k] = NPs whose distance from the droplet centre falls in shell
  * k and conc[k] = (hist[k]/N) / (dV_k / V), the normalised concentration of Eq. 8

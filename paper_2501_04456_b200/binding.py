@@ -24,6 +24,8 @@ DBG_KEYS, DBG_KEYS_SORTED, DBG_PERM, DBG_CELL_OFFSETS, DBG_IDS_SORTED, DBG_GRID 
 E_NONFINITE = -5
 E_CAPACITY = -7
 OPT_SORT, OPT_FORCE_KERNEL, OPT_TILE_SUBSTREAMS, OPT_TILE_SPAN, OPT_LIST_LANES = 1, 2, 3, 4, 5
+NOALLOC_MAX_BINS = 4096          # LV_NOALLOC_MAX_BINS: bins of the static scratch of lv_observe_rdf_noalloc
+E_CAPACITY = -7
 SORT_COUNTING, SORT_RADIX = 0, 1
 FORCE_SIMPLE, FORCE_QUEUED, FORCE_SEGMENTS, FORCE_PACKED, FORCE_TILE = 0, 1, 2, 3, 4
 
@@ -91,6 +93,7 @@ def load():
     L.lv_get_rebuild_count.argtypes = [vp, C.POINTER(C.c_int64)]
     L.lv_get_list_stats.argtypes = [vp, C.POINTER(C.c_int64)]
     L.lv_observe_rdf.argtypes = [vp, C.c_double, C.c_int, C.POINTER(C.c_uint64), dp]
+    L.lv_observe_rdf_noalloc.argtypes = [vp, C.c_double, C.c_int, C.POINTER(C.c_uint64), dp]
     L.lv_observe_clusters.argtypes = [vp, C.c_double, ip, C.POINTER(C.c_int64), dp,
                                       C.POINTER(C.c_int64), C.POINTER(C.c_uint64)]
     L.lv_render.argtypes = [vp, C.POINTER(LvView), vp, vp, C.c_int]
@@ -321,6 +324,17 @@ class Simulation:
         self._check(self.L.lv_observe_rdf(self.h, float(dr), int(n_bins),
                                           h.ctypes.data_as(C.POINTER(C.c_uint64)),
                                           g.ctypes.data_as(C.POINTER(C.c_double))), "lv_observe_rdf")
+        return h, g
+
+    def observe_rdf_noalloc(self, dr: float, n_bins: int):
+        """observe_rdf through the entry point whose scratch is a static device array of the
+        library (no allocation, no caller scratch; n_bins <= NOALLOC_MAX_BINS)."""
+        h = np.zeros(int(n_bins), dtype=np.uint64)
+        g = np.zeros(int(n_bins))
+        self._check(self.L.lv_observe_rdf_noalloc(self.h, float(dr), int(n_bins),
+                                                  h.ctypes.data_as(C.POINTER(C.c_uint64)),
+                                                  g.ctypes.data_as(C.POINTER(C.c_double))),
+                    "lv_observe_rdf_noalloc")
         return h, g
 
     def observe_radial(self, dr: float, n_bins: int):

@@ -1203,7 +1203,7 @@ const char *lv_strerror(int code)
     case LV_E_ARG: return "bad argument";
     case LV_E_ORDER: return "call order violated";
     case LV_E_WORKSPACE: return "workspace too small or misaligned";
-    case LV_E_CAPACITY: return "skin neighbour list pool exceeded (reserved; a warning since 0.2: those steps use the cells)";
+    case LV_E_CAPACITY: return "size beyond a fixed maximum of the library (lv_observe_rdf_noalloc: LV_NOALLOC_MAX_BINS)";
     case LV_E_CUDA: return "CUDA runtime error";
     case LV_E_NONFINITE: return "non-finite position or velocity";
     case LV_E_NOMEM: return "host allocation failed";
@@ -1347,3 +1347,71 @@ int lv_batch_step(lv_batch *b, int n)
 }
 
 }  // extern "C"
+
+// ---- one entry point that allocates nothing and needs no caller scratch ------------------
+// lv_observe_rdf_noalloc: the RDF pair walk (k_rdf_hist) with its histogram scratch in a
+// file-scope device array instead of the caller's workspace.  The array's name is a host-side
+// stand-in in host code: its device address is taken once per device, with that device current,
+// by cudaGetSymbolAddress, and THAT pointer goes to the kernel.  Every GPU that loads the
+// library holds the array (LV_NOALLOC_MAX_BINS * 8 bytes = 32 KiB) until the process exits.
+static __device__ __align__(256) unsigned long long g_rdf_scratch[LV_NOALLOC_MAX_BINS];
+
+namespace {
+constexpr int kMaxDevices = 64;
+unsigned long long *g_rdf_scratch_ptr[kMaxDevices];     // device address per device; nullptr: not taken yet
+
+// device address of g_rdf_scratch on the CURRENT device
+int rdf_scratch_of_current_device(lv_sim *s, unsigned long long **out)
+{
+    int dev = -1;
+    LV_CUDA(s, cudaGetDevice(&dev));
+    if (dev < 0 || dev >= kMaxDevices) return LV_E_ARG;
+    if (!g_rdf_scratch_ptr[dev]) {
+        unsigned long long *p = nullptr;
+        LV_CUDA(s, cudaGetSymbolAddress((void **)&p, g_rdf_scratch));
+        if (!p) return LV_E_CUDA;
+        g_rdf_scratch_ptr[dev] = p;      // (two threads racing here store the same address)
+    }
+    *out = g_rdf_scratch_ptr[dev];
+    return LV_OK;
+}
+}  // namespace
+
+extern "C" int lv_observe_rdf_noalloc(lv_sim *s, double dr, int n_bins, uint64_t *hist, double *g)
+{
+    if (!s || !(dr > 0.0) || n_bins < 1) return LV_E_ARG;
+    if (n_bins > LV_NOALLOC_MAX_BINS) {
+        fprintf(stderr, "lv_observe_rdf_noalloc: n_bins = %d exceeds LV_NOALLOC_MAX_BINS = %d "
+                        "(the static scratch array); use lv_observe_rdf\n", n_bins, LV_NOALLOC_MAX_BINS);
+        return LV_E_CAPACITY;
+    }
+    if (!s->bound || !s->state_set) return LV_E_ORDER;
+    if (hist) memset(hist, 0, 8 * (size_t)n_bins);
+    if (g) for (int k = 0; k < n_bins; ++k) g[k] = 0.0;
+    for (int b = 0; b < s->n_types; ++b)       // the pair walk keeps its stencil half-width in an int8
+        if (std::ceil(dr * (double)n_bins * (1.0 + 1.0 / 1024.0) / s->grid.h[b]) > 100.0) return LV_E_ARG;
+    if (s->n == 0) return LV_OK;
+    unsigned long long *dh = nullptr;
+    int rc = rdf_scratch_of_current_device(s, &dh);
+    if (rc != LV_OK) return rc;
+    // cell structures of the current state (steps (i) of PAPER.md:64), then the pair walk
+    for (int k = 0; k < 3; ++k) {
+        rc = enqueue_stage(s, k);
+        if (rc != LV_OK) return rc;
+    }
+    // the array keeps the last call's counts: the kernel adds, so it must start at zero
+    LV_CUDA(s, cudaMemsetAsync(dh, 0, 8 * (size_t)n_bins, s->stream));
+    LV_CUDA(s, lvk_rdf_hist(s->dev, s->bufs, s->grid.h, dr, n_bins, dh, s->stream));
+    uint64_t stack_hist[LV_NOALLOC_MAX_BINS];                      // 32 KiB of host stack, no heap either
+    uint64_t *hh = hist ? hist : stack_hist;
+    LV_CUDA(s, cudaMemcpyAsync(hh, dh, 8 * (size_t)n_bins, cudaMemcpyDeviceToHost, s->stream));
+    LV_CUDA(s, cudaStreamSynchronize(s->stream));
+    LvDevState st;
+    LV_CUDA(s, cudaMemcpy(&st, s->bufs.st, sizeof(st), cudaMemcpyDeviceToHost));
+    // Eq. 6: g_k = (psi_k / N) / ((N - 1) dV_k / V), V the droplet volume at this step
+    const double R = lv_radius_of(s->sched_mode, s->R0, s->R1, s->sched_steps, st.step);
+    const double V = 4.0 / 3.0 * M_PI * R * R * R, N = (double)s->n;
+    if (g && s->n > 1)
+        for (int k = 0; k < n_bins; ++k) g[k] = ((double)hh[k] / N) / ((N - 1.0) * shell_volume(k, dr) / V);
+    return LV_OK;
+}
