@@ -32,7 +32,7 @@ FORCE_SIMPLE, FORCE_QUEUED, FORCE_SEGMENTS, FORCE_PACKED, FORCE_TILE = 0, 1, 2, 
 # every symbol include/lv.h declares (tests check the library exports them all)
 SYMBOLS = ["lv_langevin_coeffs", "lv_create", "lv_set_types", "lv_set_forces",
            "lv_set_droplet_schedule", "lv_set_grid", "lv_set_option", "lv_set_neighbour_list",
-           "lv_get_rebuild_count", "lv_get_list_stats", "lv_observe_rdf", "lv_observe_radial", "lv_observe_clusters", "lv_render", "lv_render_surface", "lv_workspace_bytes", "lv_bind",
+           "lv_get_rebuild_count", "lv_get_list_stats", "lv_observe_rdf", "lv_observe_rdf_noalloc", "lv_observe_radial", "lv_observe_clusters", "lv_render", "lv_render_surface", "lv_workspace_bytes", "lv_bind",
            "lv_set_state", "lv_step", "lv_compute_forces", "lv_get_state", "lv_get_forces",
            "lv_get_status", "lv_get_debug", "lv_launches_per_step", "lv_step_profiled",
            "lv_stage_timing", "lv_read_stage_timing",
