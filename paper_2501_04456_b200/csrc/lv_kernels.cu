@@ -1092,8 +1092,14 @@ __device__ __forceinline__ float u01(uint32_t w)
 // read from B on the step that rebuilt and from A (in place) otherwise; an NP that has moved
 // farther than half the skin from its position at the build raises the rebuild flag of the
 // next step.
+// 16 blocks of 128 threads per SM (32 registers): the 1 954 blocks of an N = 250 000 step are ONE
+// wave of the 148 SMs; at 40 registers (12 blocks per SM) they were 1.10 waves and the tail wave
+// left the SMs idle for 46 % of the kernel (ncu: sm__cycles_active 11.4 k of 21.1 k cycles)
+#ifndef LV_UPD_MINB
+#define LV_UPD_MINB 16
+#endif
 template <bool kHash, bool kList>
-__global__ void __launch_bounds__(kThreads)
+__global__ void __launch_bounds__(kThreads, LV_UPD_MINB)
 k_update(const __grid_constant__ LvDev P, const float4 *__restrict__ posB_,
          const float4 *__restrict__ velB_, const float4 *__restrict__ force,
          float4 *posA, float4 *velA, LvDevState *st,
