@@ -572,7 +572,10 @@ k_pair_force_s(const __grid_constant__ LvDev P, const float4 *__restrict__ pos,
         if (gtid == 0) { *LA.scan_ticket = 0u; LA.cnt[P.n] = 0u; }
     }
     // fill modes: the NP's own list (start = exclusive scan of the reserved lengths), written
-    // four entries (16 bytes) at a time; cap = its reserve (exact build: its counted length)
+    // four entries (16 bytes) at a time from a register buffer with selects and ONE predicated
+    // store per candidate -- no divergent branch in the walk (the fill is bound by instructions;
+    // 4-byte stores, three instructions per candidate, made it L2-bound instead: 189 M sector
+    // writes); cap = its reserve (exact build: its counted length)
     uint4 *col = nullptr;
     int cap = 0;
     if (kFill && gtid < P.n) {
@@ -623,17 +626,15 @@ k_pair_force_s(const __grid_constant__ LvDev P, const float4 *__restrict__ pos,
                 const float r2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
                 const bool in = r2 < rc2 && jj[u] != self;           // fp32 contract #2
                 if (kList) {
-                    if (in) {
-                        if (!kCount) {
-                            const int q = cnt & 3;
-                            ebuf.x = q == 0 ? jj[u] : ebuf.x;
-                            ebuf.y = q == 1 ? jj[u] : ebuf.y;
-                            ebuf.z = q == 2 ? jj[u] : ebuf.z;
-                            ebuf.w = jj[u];
-                            if (q == 3 && cnt < cap) col[cnt >> 2] = ebuf;     // cap is a multiple of 4
-                        }
-                        ++cnt;
+                    if (!kCount) {
+                        const int q = cnt & 3;
+                        ebuf.x = (in && q == 0) ? jj[u] : ebuf.x;
+                        ebuf.y = (in && q == 1) ? jj[u] : ebuf.y;
+                        ebuf.z = (in && q == 2) ? jj[u] : ebuf.z;
+                        ebuf.w = in ? jj[u] : ebuf.w;
+                        if (in && q == 3 && cnt < cap) col[cnt >> 2] = ebuf;     // cap is a multiple of 4
                     }
+                    cnt += in ? 1 : 0;
                     continue;
                 }
                 const float rinv = rsqrt_approx(r2);
